@@ -1,0 +1,158 @@
+/*
+ * art_decode.h -- C ABI of the B200 (sm_100a) ART decode-attention library.
+ *
+ * ART = Attention Run-time Termination, arXiv 2606.00024.  Citations are
+ * "PAPER.md:<line>" (the extracted paper text) plus section / equation.
+ *
+ * What one call computes (Eq. 1; Algorithm 1;
+ * PAPER.md:144 Eq. 2; Eq. 3; PAPER.md:171-173 traversal orders):
+ * for every query group (sequence b, KV head g) = the G = Hq/Hkv query heads that
+ * share one KV head, walk the eligible 64-token KV blocks in the policy's traversal
+ * order; per block compute s = q k^T / sqrt(d), the online-softmax update and P V;
+ * after each block evaluate the stability criterion on the probe x^(t) of the
+ * NORMALISED intermediate output,
+ *     d_scale = ||x^(t) - x^(t-1)||_2 < tau   and   d_direction = 1 - cos(x^(t), x^(t-1)) < phi
+ * for ALL heads of the group, count consecutive stable steps, and stop loading KV
+ * blocks once the count reaches `patience`.  out = o^(t*), stop_block = t*.
+ * The readings taken where the paper is silent (probe = coordinates k*(d/32),
+ * AND over heads, sink block first, zero-norm => d_direction = 1, strict '<') are
+ * listed in DESIGN.md, "Readings".
+ *
+ * All functions are re-entrant; the library keeps no global mutable state, never
+ * allocates or frees device memory, and never retains a pointer after returning.
+ * Nothing here falls back to the CPU: on a device that is not sm_100 the calls
+ * return ART_ERR_ARCH.
+ */
+#ifndef ART_DECODE_H_
+#define ART_DECODE_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ART_VERSION 100          /* 0.1.0 */
+#define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
+#define ART_PATIENCE_INF 2147483647 /* "p = infinity": detector runs, never fires (App. E) */
+
+/* status codes: 0 = OK, negative = error.  No exceptions, no abort. */
+enum {
+  ART_OK = 0,
+  ART_ERR_NULL = -1,      /* a required pointer is NULL */
+  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G not in {1,2,4,8}, unsupported head_dim, block_tokens != 64,
+                             negative sizes, policy/list mismatch, bad thresholds */
+  ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128) */
+  ART_ERR_ALIGN = -4,     /* q / k_cache / v_cache not 16-byte aligned */
+  ART_ERR_WORKSPACE = -5, /* workspace NULL or too small for the *_host entry points */
+  ART_ERR_ARCH = -6,      /* current device is not compute capability 10.x */
+  ART_ERR_CUDA = -7       /* a CUDA runtime call or the launch failed */
+};
+
+enum { ART_DTYPE_F32 = 0, ART_DTYPE_BF16 = 1 };          /* element type of q, k_cache, v_cache */
+enum { ART_LAYOUT_HND = 0,  /* cache[page][kv_head][token][d]: one contiguous 16 KiB tile per (page, head) */
+       ART_LAYOUT_NHD = 1 };/* cache[page][token][kv_head][d] */
+enum { ART_POLICY_DENSE = 0,        /* all blocks, most recent first */
+       ART_POLICY_SINK_WINDOW = 1,  /* tokens {j < sink} U {j >= L - window}; block 0 first, then
+                                       descending (reading R3) */
+       ART_POLICY_LIST = 2 };       /* eligible_blocks walked in the order given */
+
+/* Problem description.  HOST memory, read during the call only. */
+typedef struct art_desc {
+  int32_t batch;               /* B */
+  int32_t num_q_heads;         /* Hq */
+  int32_t num_kv_heads;        /* Hkv; query head h uses KV head h / (Hq/Hkv) */
+  int32_t head_dim;            /* d: 64 (F32) or 128 (BF16) */
+  int32_t block_tokens;        /* must be 64 */
+  int32_t dtype;               /* ART_DTYPE_* */
+  int32_t kv_layout;           /* ART_LAYOUT_* */
+  int32_t policy;              /* ART_POLICY_* */
+  int32_t max_blocks_per_seq;  /* row stride of block_table */
+  int32_t sink_tokens;         /* SINK_WINDOW */
+  int32_t window_tokens;       /* SINK_WINDOW */
+  int32_t max_eligible;        /* row stride of eligible_blocks (LIST) */
+  float sm_scale;              /* logit scale; 0 => 1/sqrt(d) (Eq. 1) */
+  int32_t split;               /* CTAs (thread-block cluster size) cooperating on one group:
+                                  0 = choose automatically, else 1, 2, 4, 8 or 16.  Any value gives the
+                                  same stop_block as the sequential algorithm. */
+  const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
+  int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
+                                  (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */
+} art_desc_t;
+
+/* Termination thresholds (tau = 1e-5, phi = 1e-3, p = 5).  HOST memory. */
+typedef struct art_thresholds {
+  float tau;          /* scale tolerance, compared as d_scale < tau (strict) */
+  float phi;          /* direction tolerance, d_direction < phi (strict) */
+  int32_t patience;   /* p >= 1; ART_PATIENCE_INF never fires */
+  int32_t probe_dim;  /* m: 32 = coordinates k*(d/32) (default); 0 or d = all coordinates */
+} art_thresholds_t;
+
+/*
+ * ART-on decode attention.  Enqueues on `cuda_stream` (a cudaStream_t, NULL = default
+ * stream) and returns; results are valid once the stream has been synchronised.
+ *
+ *   q               DEVICE [B, Hq, d]            dtype elements, 16-B aligned
+ *   k_cache,v_cache DEVICE paged caches (kv_layout), dtype elements, 16-B aligned
+ *   block_table     DEVICE int32 [B, max_blocks_per_seq]  logical block -> physical page
+ *   eligible_blocks DEVICE int32 [B, Hkv, max_eligible]   LOGICAL block ids, distinct, walked in the
+ *                   order given; NULL unless policy == LIST
+ *   seq_lens        DEVICE int32 [B]; tokens >= seq_lens[b] of the last block are masked
+ *   thresholds      HOST
+ *   out             DEVICE float32 [B, Hq, d]    o^(t*) (Alg. 1 l.18)
+ *   stop_block      DEVICE int32 [B, Hkv]        t* = number of blocks processed, in [0, T];
+ *                                                T if the criterion never fired
+ *   workspace       unused by this entry point (may be NULL)
+ *
+ * seq_lens[b] == 0 or an empty list gives a zero output row and stop_block 0.
+ * Device-side contents (page ids in range, list entries valid) are not validated.
+ */
+int art_decode_attention(const art_desc_t* desc, const void* q, const void* k_cache,
+                         const void* v_cache, const int32_t* block_table,
+                         const int32_t* eligible_blocks, const int32_t* seq_lens,
+                         const art_thresholds_t* thresholds, float* out, int32_t* stop_block,
+                         void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * ART-off: the same kernel source with the detector compiled out (NOT "patience = inf").
+ * out = o^(T) (Eq. 1 over the eligible tokens); stop_block[b, g] = T.
+ */
+int art_decode_attention_off(const art_desc_t* desc, const void* q, const void* k_cache,
+                             const void* v_cache, const int32_t* block_table,
+                             const int32_t* eligible_blocks, const int32_t* seq_lens,
+                             float* out, int32_t* stop_block,
+                             void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * End-to-end variants for a serving loop: the per-step inputs (q, block_table,
+ * eligible_blocks, eligible_counts, seq_lens) are HOST buffers (pinned for async
+ * copies), copied to the device inside the call; out and stop_block are HOST buffers
+ * filled before the call returns (the call synchronises the stream).  The KV caches
+ * are decode STATE and stay DEVICE pointers.  desc->eligible_counts is then a HOST
+ * pointer; desc->blocks_loaded must be NULL.  `thresholds == NULL` selects ART-off.
+ * `workspace` is DEVICE scratch of at least art_workspace_bytes(desc).
+ */
+int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const void* k_cache,
+                              const void* v_cache, const int32_t* block_table_host,
+                              const int32_t* eligible_blocks_host, const int32_t* seq_lens_host,
+                              const art_thresholds_t* thresholds, float* out_host,
+                              int32_t* stop_block_host, void* workspace, size_t workspace_bytes,
+                              void* cuda_stream);
+
+/* DEVICE scratch bytes art_decode_attention_host needs for this problem (0 on a bad desc). */
+size_t art_workspace_bytes(const art_desc_t* desc);
+
+/* Cluster size the library would pick for desc->split == 0 (needs a CUDA device); <0 = error code. */
+int art_query_split(const art_desc_t* desc, int art_on);
+
+/* Human-readable text for a status code (static storage). */
+const char* art_status_string(int status);
+
+/* ART_VERSION of the loaded library. */
+int art_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ART_DECODE_H_ */
