@@ -1,0 +1,384 @@
+#!/usr/bin/env python
+"""bench.py -- ART decode-attention benchmark (contract in the task prompt).
+
+One "step" = one pass of the whole hot path (resolve blocks, TMA loads, scores, online softmax,
+P.V, probe + criterion + patience, early exit, finalise) over one decode batch of synthetic input.
+At N = 1 the workload is BASELINE.json configs[1] (Mistral-7B-shaped decode layer: batch 8,
+Hq 32 / Hkv 8, d 128, context 32768, bf16 paged KV, dense policy, paper-default thresholds).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W]          # this repo's CUDA path
+    python bench.py --impl reference ...                          # the CPU oracle, as it stands
+    python bench.py --report                                       # all five configs (+ variants), one JSON line each
+
+Prints ONE JSON line (rank 0).  `value` is KV tokens/s (sum over sequences of eligible tokens per
+step / step time) with inputs resident in HBM; `e2e` is the same through art_decode_attention_host
+with pinned HOST q / tables / outputs copied inside the timed region (the KV cache is decode state
+and stays in HBM).  Multi-GPU: the path shards by sequence with no exchange, so every rank runs its
+own configs[1]-shaped batch (weak scaling) and no data-path collective exists.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "art_decode_attn_kv_tokens_per_s"
+UNIT = "KV tok/s"
+BLOCK_BYTES = 32768                      # K + V of one 64-token block of one KV head
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def committed_traffic():
+    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f)
+    return {}
+
+
+class ClockSampler:
+    """Samples SM clock and throttle reasons DURING the timed region (NVML)."""
+    REASONS = {0x4: "sw_power_cap", 0x8: "hw_slowdown", 0x20: "sw_thermal_slowdown",
+               0x40: "hw_thermal_slowdown", 0x80: "hw_power_brake_slowdown"}
+
+    def __init__(self, index: int):
+        self.samples, self.reasons, self.max_mhz, self._stop = [], set(), None, threading.Event()
+        self._h = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self._h = None
+        self._t = threading.Thread(target=self._run, daemon=True)
+
+    def _run(self):
+        while not self._stop.is_set() and self._h is not None:
+            try:
+                self.samples.append(int(self._nv.nvmlDeviceGetClockInfo(self._h, self._nv.NVML_CLOCK_SM)))
+                r = int(self._nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                for bit, name in self.REASONS.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(0.02)
+
+    def __enter__(self):
+        self._t.start(); return self
+
+    def __exit__(self, *a):
+        self._stop.set(); self._t.join(timeout=1.0)
+
+    def summary(self):
+        s = sorted(self.samples)
+        return {"sm_mhz": (s[len(s) // 2] if s else None), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(s)}
+
+
+def eligible_tokens(w) -> int:
+    """Sum over sequences of eligible tokens (sequence level, not multiplied by Hkv)."""
+    import torch
+    from workloads import generators as gen
+    L = w.seq_lens.to(torch.int64)
+    if w.policy == gen.POLICY_DENSE:
+        return int(L.sum())
+    if w.policy == gen.POLICY_SINK_WINDOW:
+        s = torch.minimum(L, torch.tensor(w.sink_tokens, device=L.device))
+        win = torch.minimum(L, torch.tensor(w.window_tokens, device=L.device))
+        return int(torch.minimum(L, s + win).sum())
+    # LIST: tokens of the listed blocks, averaged over the KV heads of a sequence
+    cnt = w.eligible_counts.to(torch.int64)
+    blk = w.eligible_blocks.to(torch.int64)
+    idx = torch.arange(blk.shape[2], device=blk.device)[None, None, :] < cnt[:, :, None]
+    tok = torch.clamp(L[:, None, None] - blk * 64, min=0, max=64) * idx
+    return int(tok.sum() // w.num_kv_heads)
+
+
+def time_loop(fn, steps: int, warmup: int, barrier=None):
+    """W untimed steps, then exactly K steps between CUDA events on the current stream."""
+    import torch
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    return e0.elapsed_time(e1)            # ms for K steps
+
+
+def make_runner(art, w, *, art_on: bool, split: int = 0, **th):
+    """Pre-marshalled call (descriptors and outputs allocated once); returns (fn, out, stop, loaded)."""
+    import torch
+    dev = w.q.device
+    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32, device=dev)
+    stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev)
+    loaded = torch.zeros((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev)
+    desc = art.make_desc(w, split=split, blocks_loaded=loaded)
+    thr = art.ArtThresholds(tau=th.get("tau", w.tau), phi=th.get("phi", w.phi),
+                            patience=th.get("patience", w.patience), probe_dim=th.get("probe_dim", w.probe_dim))
+    if art_on:
+        fn = lambda: art.art_decode_attention(desc, w.q, w.k_cache, w.v_cache, w.block_table, w.eligible_blocks,
+                                              w.seq_lens, thr, out, stop)
+    else:
+        fn = lambda: art.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table,
+                                                  w.eligible_blocks, w.seq_lens, out, stop)
+    return fn, out, stop, loaded
+
+
+def make_host_runner(art, w, *, art_on: bool):
+    """art_decode_attention_host: per-step inputs / outputs in pinned host memory."""
+    import torch
+    pin = lambda t: None if t is None else t.cpu().pin_memory()
+    q, bt, sl, el, ec = pin(w.q), pin(w.block_table), pin(w.seq_lens), pin(w.eligible_blocks), pin(w.eligible_counts)
+    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32).pin_memory()
+    stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32).pin_memory()
+    desc = art.make_desc(w, eligible_counts=ec)
+    ws = torch.empty(art.art_workspace_bytes(desc), dtype=torch.uint8, device=w.q.device)
+    thr = art.ArtThresholds(tau=w.tau, phi=w.phi, patience=w.patience, probe_dim=w.probe_dim) if art_on else None
+    fn = lambda: art.art_decode_attention_host(desc, q, w.k_cache, w.v_cache, bt, el, sl, thr, out, stop, ws)
+    nbytes = lambda t: 0 if t is None else t.numel() * t.element_size()
+    h2d = nbytes(q) + nbytes(bt) + nbytes(sl) + nbytes(el) + nbytes(ec)
+    d2h = nbytes(out) + nbytes(stop)
+    return fn, h2d, d2h, (q, bt, sl, el, ec, out, stop, ws)
+
+
+def measure(art, w, steps, warmup, barrier=None, *, art_on=True, split=0, **th):
+    """Times one configuration; returns a dict of per-step numbers."""
+    fn, out, stop, loaded = make_runner(art, w, art_on=art_on, split=split, **th)
+    ms = time_loop(fn, steps, warmup, barrier)
+    us = ms * 1e3 / steps
+    processed = int(stop.sum())
+    ld = int(loaded.sum())
+    return {"us_per_step": us, "blocks_processed": processed, "blocks_loaded": ld,
+            "gbs_processed": processed * BLOCK_BYTES / (us * 1e-6) / 1e9,
+            "gbs_loaded": ld * BLOCK_BYTES / (us * 1e-6) / 1e9, "ms_total": ms}
+
+
+def oracle_sample(w, n_groups: int, art_on: bool = True):
+    """The CPU oracle, as it stands, on a bounded sample of groups of workload w (single BLAS thread).
+    Returns (seconds, sequence-level KV tokens covered, threads)."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import extract_groups, run_oracle       # imports oracle/: cpu_baseline leg only
+    import numpy as np
+    rng = np.random.default_rng(0)
+    B, Hkv = w.batch, w.num_kv_heads
+    groups = [(int(rng.integers(B)), int(rng.integers(Hkv))) for _ in range(n_groups)]
+    mini = extract_groups(w, groups)
+    try:
+        from threadpoolctl import threadpool_limits
+        ctx = threadpool_limits(limits=1)
+    except Exception:
+        import contextlib
+        ctx = contextlib.nullcontext()
+    tokens_all = eligible_tokens(mini)                   # mini has Hkv = 1: per-group tokens
+    with ctx:
+        t0 = time.perf_counter()
+        run_oracle(mini, art=art_on)
+        dt = time.perf_counter() - t0
+    return dt, tokens_all / Hkv, 1
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle timed on host cores, bounded sample per step."""
+    if rank != 0:
+        return
+    import torch
+    from workloads import generators as gen
+    w = gen.config(1, device="cpu", batch=1)             # one sequence of configs[1]; groups sampled from it
+    n_groups = 2
+    times = []
+    for i in range(args.warmup + args.steps):
+        dt, toks, cores = oracle_sample(w, n_groups)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * sum(times) / len(times)
+    val = toks / (ms * 1e-3)
+    sample = f"{n_groups} of 64 (sequence, KV-head) groups of configs[1] per step (context 32768, G=4, d=128)"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": "configs[1] mistral7b-shaped decode layer (bounded sample)", "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def run_report(args):
+    """All five configs (+ variants R / 0c), ART-on / ART-off / p = inf; one JSON line per row."""
+    import torch
+    from workloads import generators as gen
+    import paper_2606_00024_b200 as art
+    peak, which = peaks()
+    rows = [(0, "a", ""), (0, "a", "c"), (1, "a", ""), (1, "a", "R"), (2, "a", ""), (2, "a", "R"),
+            (3, "a", ""), (3, "a", "R"), (3, "b", ""), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
+    for index, sub, variant in rows:
+        w = gen.config(index, sub=sub, variant=variant, device="cuda")
+        torch.cuda.synchronize()
+        toks = eligible_tokens(w)
+        off = measure(art, w, args.steps, args.warmup, art_on=False)
+        on = measure(art, w, args.steps, args.warmup, art_on=True)
+        pinf = measure(art, w, args.steps, args.warmup, art_on=True, patience=art.ART_PATIENCE_INF)
+        total_blocks = off["blocks_processed"]
+        row = {"workload": w.name, "groups": w.batch * w.num_kv_heads, "split_on": art.art_query_split(art.make_desc(w), True),
+               "eligible_tokens": toks, "blocks_total": total_blocks,
+               "off_us": round(off["us_per_step"], 2), "off_gbs": round(off["gbs_processed"], 1),
+               "off_frac_of_peak": round(off["gbs_processed"] / peak, 4),
+               "on_us": round(on["us_per_step"], 2), "on_gbs_loaded": round(on["gbs_loaded"], 1),
+               "on_frac_of_peak_loaded": round(on["gbs_loaded"] / peak, 4),
+               "on_gbs_processed": round(on["gbs_processed"], 1),
+               "skipped_frac": round(1 - on["blocks_processed"] / max(total_blocks, 1), 4),
+               "loaded_frac": round(on["blocks_loaded"] / max(total_blocks, 1), 4),
+               "speedup_on_vs_off": round(off["us_per_step"] / on["us_per_step"], 4),
+               "pinf_overhead": round(pinf["us_per_step"] / off["us_per_step"] - 1, 4),
+               "kv_tok_s_on": toks / (on["us_per_step"] * 1e-6), "kv_tok_s_off": toks / (off["us_per_step"] * 1e-6),
+               "peak_gbs": peak, "peak_kind": which}
+        print(json.dumps(row), flush=True)
+        del w
+        torch.cuda.empty_cache()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="art", choices=["art", "reference"])
+    ap.add_argument("--report", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "art" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if args.report:
+        run_report(args)
+        return
+
+    import torch
+    import torch.distributed as dist
+    from workloads import generators as gen
+    import paper_2606_00024_b200 as art           # raises if the CUDA library is not built: no fallback
+
+    torch.cuda.set_device(local)
+    barrier = None
+    if world > 1:
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        barrier = dist.barrier
+    dev = torch.device("cuda", local)
+
+    # configs[1]; every rank its own batch (seed offset), no exchange between ranks
+    w = gen.config(1, device=dev, seed=gen.SEED_BASE + 1000 + 17 * rank)
+    wR = gen.config(1, device=dev, variant="R", seed=gen.SEED_BASE + 1000 + 17 * rank)
+    torch.cuda.synchronize()
+    toks = eligible_tokens(w)
+    peak, which = peaks()
+
+    # ---- the timed region of the contract: exactly K ART-on steps on the literal config
+    fn, out, stop, loaded = make_runner(art, w, art_on=True)
+    with ClockSampler(local) as cs:
+        ms = time_loop(fn, args.steps, args.warmup, barrier)
+    clocks = cs.summary()
+    t = torch.tensor([ms], dtype=torch.float64, device=dev)
+    tk = torch.tensor([float(toks)], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tk, op=dist.ReduceOp.SUM)
+    ms_max, toks_all = float(t), float(tk)
+    ms_per_step = ms_max / args.steps
+    value = toks_all / (ms_per_step * 1e-3)
+    processed, ld = int(stop.sum()), int(loaded.sum())
+
+    # ---- end to end through the host entry point (H2D of q / tables, D2H of out / stop inside)
+    hfn, h2d, d2h, _keep = make_host_runner(art, w, art_on=True)
+    for _ in range(args.warmup):
+        hfn()
+    torch.cuda.synchronize()
+    if barrier:
+        barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        hfn()                                  # synchronises the stream itself
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_value = toks_all / (float(te) / args.steps * 1e-3)
+
+    # ---- context numbers (outside the contract's timed region): ART-off, p = inf, variant R
+    off = measure(art, w, args.steps, args.warmup, barrier, art_on=False)
+    pinf = measure(art, w, args.steps, args.warmup, barrier, art_on=True, patience=art.ART_PATIENCE_INF)
+    r_off = measure(art, wR, args.steps, args.warmup, barrier, art_on=False)
+    r_on = measure(art, wR, args.steps, args.warmup, barrier, art_on=True)
+
+    if rank == 0:
+        us = ms / args.steps * 1e3             # this rank's own kernel time per launch
+        achieved = ld * BLOCK_BYTES / (us * 1e-6) / 1e9
+        traffic = committed_traffic().get("art_on_cfg1_dram_bytes_per_launch")
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "bf16 KV, f32 accumulate", "data": "synthetic",
+            "config": {"workload": "configs[1] mistral7b-shaped decode layer: batch 8, Hq 32, Hkv 8, d 128, "
+                                   "context 32768, bf16 paged KV (64-token pages, permuted), dense policy, "
+                                   "tau 1e-5 phi 1e-3 p 5 (ART on)",
+                       "l2": "inputs larger than L2: 1 GiB of KV streamed per step vs 126 MB L2",
+                       "cluster_size": art.art_query_split(art.make_desc(w), True), "per_gpu_batch": w.batch},
+            "clocks": clocks,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h},
+            "gpu_launches": args.steps,
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                         "frac": achieved / peak, "traffic": traffic, "peak_kind": which,
+                         "kernel": "art_decode_kernel<bf16,128,G=4,ART on>",
+                         "bytes_per_launch": ld * BLOCK_BYTES, "frac_of_nominal_8TBs": achieved / 8000.0},
+            "art": {"on_us_per_step": us, "off_us_per_step": off["us_per_step"],
+                    "off_gbs": off["gbs_processed"], "off_frac_of_peak": off["gbs_processed"] / peak,
+                    "pinf_overhead": pinf["us_per_step"] / off["us_per_step"] - 1.0,
+                    "skipped_frac": 1.0 - processed / max(off["blocks_processed"], 1),
+                    "speedup_on_vs_off": off["us_per_step"] / us,
+                    "variant_R": {"on_us_per_step": r_on["us_per_step"], "off_us_per_step": r_off["us_per_step"],
+                                  "speedup_on_vs_off": r_off["us_per_step"] / r_on["us_per_step"],
+                                  "skipped_frac": 1.0 - r_on["blocks_processed"] / max(r_off["blocks_processed"], 1),
+                                  "loaded_frac": r_on["blocks_loaded"] / max(r_off["blocks_processed"], 1),
+                                  "on_gbs_loaded": r_on["gbs_loaded"], "on_frac_of_peak_loaded": r_on["gbs_loaded"] / peak}},
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            dt, ctoks, cores = oracle_sample(w, 16)
+            line["cpu_baseline"] = {"value": ctoks / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": "16 of 64 (sequence, KV-head) groups of configs[1], one pass, ART on"}
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

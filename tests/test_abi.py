@@ -1,0 +1,87 @@
+"""CPU: the C-ABI library loads, exports every symbol include/art_decode.h declares, and validates
+its arguments before touching CUDA (no compute calls without a GPU)."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def art():
+    from paper_2606_00024_b200 import build
+    build.build()
+    import paper_2606_00024_b200 as a
+    return a
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "art_decode.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(art_[a-z_]+)\s*\(", text)))
+
+
+def test_every_declared_symbol_is_exported(art):
+    lib = art.load_library()
+    syms = declared_symbols()
+    assert {"art_decode_attention", "art_decode_attention_off", "art_decode_attention_host",
+            "art_workspace_bytes", "art_query_split", "art_status_string", "art_version"} <= set(syms)
+    for s in syms:
+        assert hasattr(lib, s), s
+    assert art.art_version() == 100
+    assert "NULL" in art.art_status_string(-1) and art.art_status_string(0) == "ok"
+
+
+def test_struct_layout_matches_header(art):
+    assert C.sizeof(art.ArtDesc) == 72 and art.ArtDesc.eligible_counts.offset == 56
+    assert C.sizeof(art.ArtThresholds) == 16
+
+
+def _call_off(art, desc, q=16, k=32, v=48, bt=64, el=None, sl=80, out=96, stop=112):
+    lib = art.load_library()
+    vp = lambda x: None if x is None else C.c_void_p(x)
+    return lib.art_decode_attention_off(C.byref(desc), vp(q), vp(k), vp(v), vp(bt), vp(el), vp(sl), vp(out), vp(stop),
+                                        None, 0, None)
+
+
+def good_desc(art, **kw):
+    d = dict(batch=2, num_q_heads=8, num_kv_heads=2, head_dim=128, block_tokens=64, dtype=art.ART_DTYPE_BF16,
+             kv_layout=0, policy=0, max_blocks_per_seq=4)
+    d.update(kw)
+    return art.ArtDesc(**d)
+
+
+def test_argument_validation_happens_before_cuda(art):
+    """Fake (never dereferenced) pointers: every error below is decided on the host."""
+    assert _call_off(art, good_desc(art), q=None) == -1                      # ART_ERR_NULL
+    assert _call_off(art, good_desc(art, num_q_heads=7)) == -2               # Hq % Hkv
+    assert _call_off(art, good_desc(art, num_q_heads=32, num_kv_heads=2)) == -2   # G = 16 unsupported
+    assert _call_off(art, good_desc(art, block_tokens=32)) == -2
+    assert _call_off(art, good_desc(art, head_dim=96)) == -2
+    assert _call_off(art, good_desc(art, head_dim=64)) == -3                 # bf16 d=64 not built
+    assert _call_off(art, good_desc(art, dtype=5)) == -3
+    assert _call_off(art, good_desc(art, policy=2)) == -1                    # LIST without a list
+    assert _call_off(art, good_desc(art, policy=1, sink_tokens=-1)) == -2
+    assert _call_off(art, good_desc(art, split=3)) == -2
+    assert _call_off(art, good_desc(art), k=33) == -4                        # ART_ERR_ALIGN
+    lib = art.load_library()
+    th = art.ArtThresholds(tau=1e-5, phi=1e-3, patience=0, probe_dim=32)
+    vp = C.c_void_p
+    rc = lib.art_decode_attention(C.byref(good_desc(art)), vp(16), vp(32), vp(48), vp(64), None, vp(80), C.byref(th),
+                                  vp(96), vp(112), None, 0, None)
+    assert rc == -2                                                          # patience < 1
+    th = art.ArtThresholds(tau=1e-5, phi=1e-3, patience=5, probe_dim=48)
+    rc = lib.art_decode_attention(C.byref(good_desc(art)), vp(16), vp(32), vp(48), vp(64), None, vp(80), C.byref(th),
+                                  vp(96), vp(112), None, 0, None)
+    assert rc == -2
+
+
+def test_no_gpu_means_loud_failure_not_fallback(art):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    rc = _call_off(art, good_desc(art))
+    assert rc in (-6, -7)                                                    # ART_ERR_ARCH / ART_ERR_CUDA
+    assert art.art_workspace_bytes(good_desc(art)) > 0

@@ -1,0 +1,232 @@
+"""-m gpu: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded payload.  Sizes the oracle finishes in seconds, spanning several tiles, ragged tails
+and every policy / layout / group size; then the BASELINE-size configs on sampled groups."""
+import numpy as np
+import pytest
+import torch
+
+from workloads import generators as gen
+from parity import compare, OUT_TOL
+from helpers import extract_groups, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def art():
+    import paper_2606_00024_b200 as a
+    return a
+
+
+def f32(x):
+    return float(np.float32(x))
+
+
+def check(w, *, art_on=True, split=0, tol=None, expect_fired=None, **kw):
+    a = art()
+    wc = w.to("cuda")
+    out, stop, loaded = a.run_workload(wc, art=art_on, split=split, want_loaded=True, **kw)
+    torch.cuda.synchronize()
+    over = {k: (f32(v) if k in ("tau", "phi") else v) for k, v in kw.items()}
+    rep = compare(w, out, stop, art=art_on, oracle_over=over)
+    tol = OUT_TOL[w.dtype] if tol is None else tol
+    assert rep.stop_mismatch_nonfragile == 0, rep
+    assert rep.max_rel_err <= tol, rep
+    assert (loaded.cpu() >= stop.cpu()).all() or not art_on
+    if expect_fired is not None:
+        assert (rep.fired_groups > 0) == expect_fired, rep
+    return out, stop, loaded, rep
+
+
+# ------------------------------------------------------------------ config 0 (fp32, d = 64)
+
+@pytest.mark.parametrize("split", [0, 1, 2, 4, 8, 16])
+@pytest.mark.parametrize("variant", ["", "c"])
+def test_config0(split, variant):
+    w = gen.config(0, variant=variant)
+    out, stop, _, rep = check(w, split=split, expect_fired=(variant == "c"))
+    assert int(stop[0, 0]) == (6 if variant == "c" else 32)       # SURVEY finding F1 / variant 0c
+    check(w, art_on=False, split=split)
+
+
+# ------------------------------------------------------------------ shrunken configs 1-4 (bf16, d = 128)
+
+_CACHE = {}
+
+
+def small(index, **kw):
+    """Shrunken BASELINE configs (same recipe, shorter context, smaller batch); cached per test session."""
+    key = (index, tuple(sorted(kw.items())))
+    if key not in _CACHE:
+        scale = {1: 1 / 8, 2: 1 / 8, 3: 1 / 2, 4: 1 / 32}[index]
+        batch = {1: 2, 2: 2, 3: 4, 4: 2}[index]
+        _CACHE[key] = gen.config(index, scale=scale, batch=batch, **kw)
+    return _CACHE[key]
+
+
+@pytest.mark.parametrize("index,sub", [(1, "a"), (2, "a"), (3, "a"), (3, "b"), (4, "a")])
+@pytest.mark.parametrize("split", [0, 1, 2, 4])
+def test_small_configs_literal_and_off(index, sub, split):
+    w = small(index, sub=sub)
+    check(w, split=split)                       # paper-default thresholds: never fires on these (F1)
+    check(w, art_on=False, split=split)
+
+
+@pytest.mark.parametrize("index,sub", [(1, "a"), (2, "a"), (3, "a"), (3, "b"), (4, "a")])
+@pytest.mark.parametrize("split", [1, 2, 4, 8])
+def test_small_configs_firing(index, sub, split):
+    """Recency decay strong enough that ART fires mid-stream at these short contexts."""
+    w = small(index, sub=sub, recency_decay=(0.2, 1.0))
+    _, stop, loaded, rep = check(w, split=split, tau=1e-3, expect_fired=True)
+    assert rep.mean_stop_frac <= 1.0 and (loaded.cpu() >= stop.cpu()).all()
+
+
+@pytest.mark.parametrize("layout", [gen.LAYOUT_HND, gen.LAYOUT_NHD])
+def test_layouts_agree(layout):
+    w = small(3, sub="a", layout=layout, recency_decay=(0.2, 1.0))
+    check(w, tau=1e-3, split=2)
+
+
+@pytest.mark.parametrize("G", [1, 2, 4, 8])
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+def test_group_sizes(G, dtype):
+    d = 64 if dtype == torch.float32 else 128
+    w = gen.make_workload("g", seed=5 + G, batch=3, num_q_heads=2 * G, num_kv_heads=2, head_dim=d,
+                          seq_lens=[1000, 64, 3111], dtype=dtype, recency_decay=(0.3, 1.0))
+    check(w, tau=1e-3, split=2, expect_fired=True)
+    check(w, art_on=False, split=4)
+
+
+def test_full_probe():
+    """probe_dim = 0: the detector sees all d coordinates."""
+    for dtype, d in ((torch.bfloat16, 128), (torch.float32, 64)):
+        w = gen.make_workload("p", seed=77, batch=2, num_q_heads=8, num_kv_heads=2, head_dim=d,
+                              seq_lens=[4096, 2500], dtype=dtype, recency_decay=(0.3, 1.0))
+        check(w, tau=2e-3, probe_dim=0, split=2, expect_fired=True)
+
+
+def test_patience_inf_equals_off():
+    """App. E: detector on, never firing => same result as the baseline kernel."""
+    a = art()
+    w = small(1, recency_decay=(0.2, 1.0)); wc = w.to("cuda")
+    o1, s1, _ = a.run_workload(wc, art=True, patience=a.ART_PATIENCE_INF, split=2)
+    o0, s0, _ = a.run_workload(wc, art=False, split=2)
+    assert torch.equal(s1, s0)
+    assert torch.equal(o1, o0)                  # same fold order => bit-identical
+
+
+def test_ablation_switches_and_extremes():
+    """Table 3 switches as threshold settings: w/o d_scale (tau = inf), w/o d_direction (phi = inf),
+    w/o patience (p = 1); and tau = phi = inf, p = 1 => t* = 1."""
+    w = small(1, recency_decay=(0.2, 1.0))
+    inf = float("inf")
+    base = check(w, tau=1e-3)[1]
+    no_dir = check(w, tau=1e-3, phi=inf)[1]
+    no_pat = check(w, tau=1e-3, patience=1)[1]
+    no_scale = check(w, tau=inf)[1]
+    assert (no_dir <= base).all() and (no_pat <= base).all() and (no_scale <= base).all()
+    assert (check(w, tau=inf, phi=inf, patience=1)[1] == 1).all()
+    assert (check(w, tau=0.0)[1] == 64).all()
+
+
+def test_split_invariance_and_determinism():
+    a = art()
+    w = small(1, recency_decay=(0.2, 1.0)); wc = w.to("cuda")
+    ref_o, ref_s, _ = a.run_workload(wc, tau=1e-3, split=1)
+    for split in (1, 2, 4, 8, 16):
+        o, s, _ = a.run_workload(wc, tau=1e-3, split=split)
+        assert torch.equal(s, ref_s)
+        assert (o - ref_o).abs().max() <= 1e-5 * ref_o.abs().max()
+        o2, s2, _ = a.run_workload(wc, tau=1e-3, split=split)
+        assert torch.equal(o, o2) and torch.equal(s, s2)
+
+
+def test_edge_cases():
+    """Empty / one-token / 63-64-65-token sequences, empty window, lists with blocks beyond L,
+    empty lists; NaN in every masked slot."""
+    lens = [0, 1, 63, 64, 65, 130]
+    w = gen.make_workload("e", seed=3, batch=6, num_q_heads=8, num_kv_heads=2, head_dim=128, seq_lens=lens)
+    out, stop, _, _ = check(w, split=2)
+    assert (out[0] == 0).all() and (stop[0] == 0).all()
+    check(w, art_on=False, split=1)
+    w2 = gen.make_workload("e2", seed=4, batch=6, num_q_heads=8, num_kv_heads=2, head_dim=128, seq_lens=lens,
+                           policy=gen.POLICY_SINK_WINDOW, sink_tokens=4, window_tokens=0)
+    out, stop, _, _ = check(w2, art_on=False)
+    assert stop[:, 0].tolist() == [0, 1, 1, 1, 1, 1]
+    w3 = gen.make_workload("e3", seed=4, batch=6, num_q_heads=8, num_kv_heads=2, head_dim=128, seq_lens=lens,
+                           policy=gen.POLICY_SINK_WINDOW, sink_tokens=0, window_tokens=0)
+    out, stop, _, _ = check(w3, art_on=False)
+    assert (out == 0).all() and (stop == 0).all()
+    w4 = gen.make_workload("e4", seed=9, batch=2, num_q_heads=4, num_kv_heads=2, head_dim=128, seq_lens=[300, 100],
+                           policy=gen.POLICY_LIST, topk_blocks=3)
+    w4.eligible_blocks[0, 0] = torch.tensor([4, 9, 0])      # block 9 lies wholly beyond L: a step, no tokens
+    w4.eligible_counts[1, 1] = 0                            # empty list
+    out, stop, _, _ = check(w4, split=2)
+    assert int(stop[1, 1]) == 0 and (out[1, 2:] == 0).all()
+    check(w4, art_on=False)
+
+
+def test_error_codes_on_device():
+    a = art()
+    w = small(1).to("cuda")
+    desc = a.make_desc(w)
+    desc.head_dim = 96
+    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), device="cuda")
+    stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device="cuda")
+    with pytest.raises(a.ArtError) as e:
+        a.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table, None, w.seq_lens, out, stop)
+    assert e.value.status == -2
+    assert a.art_query_split(a.make_desc(w), True) in (1, 2, 4, 8, 16)
+
+
+def test_host_entry_point():
+    """art_decode_attention_host: pinned host inputs/outputs, KV caches on the device."""
+    a = art()
+    w = small(2, recency_decay=(0.2, 1.0)); wc = w.to("cuda")
+    counts_host = w.eligible_counts.pin_memory()            # keep alive: desc only holds the pointer
+    desc = a.make_desc(w, eligible_counts=counts_host)
+    ws = torch.empty(a.art_workspace_bytes(desc), dtype=torch.uint8, device="cuda")
+    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32).pin_memory()
+    stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32).pin_memory()
+    th = a.ArtThresholds(tau=1e-3, phi=1e-3, patience=5, probe_dim=32)
+    a.art_decode_attention_host(desc, w.q.pin_memory(), wc.k_cache, wc.v_cache, w.block_table.pin_memory(),
+                                w.eligible_blocks.pin_memory(), w.seq_lens.pin_memory(), th, out, stop, ws)
+    o_dev, s_dev, _ = a.run_workload(wc, tau=1e-3)
+    assert torch.equal(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
+    a.art_decode_attention_host(desc, w.q.pin_memory(), wc.k_cache, wc.v_cache, w.block_table.pin_memory(),
+                                w.eligible_blocks.pin_memory(), w.seq_lens.pin_memory(), None, out, stop, ws)
+    o_dev, s_dev, _ = a.run_workload(wc, art=False)
+    assert torch.equal(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
+
+
+# ------------------------------------------------------------------ BASELINE-size configs, sampled groups
+
+FULL = [(1, "a", ""), (1, "a", "R"), (2, "a", ""), (2, "a", "R"), (3, "a", "R"), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
+
+
+@pytest.mark.parametrize("index,sub,variant", FULL)
+def test_full_size_sampled(index, sub, variant):
+    """configs[1..4] at BASELINE.json's sizes, in the launch configuration bench.py times (split = 0,
+    auto), ART-on and ART-off; the oracle recomputes sampled groups one by one."""
+    a = art()
+    w = gen.config(index, sub=sub, variant=variant, device="cuda")
+    torch.cuda.synchronize()
+    rng = np.random.default_rng(index * 10 + len(variant))
+    B, Hkv = w.batch, w.num_kv_heads
+    groups = sorted({(int(rng.integers(B)), int(rng.integers(Hkv))) for _ in range(5)})
+    for art_on in (True, False):
+        out, stop, loaded = a.run_workload(w, art=art_on, want_loaded=True)
+        torch.cuda.synchronize()
+        assert torch.isfinite(out).all()
+        mini = extract_groups(w, groups)
+        o_g = torch.stack([out[b, g * w.group_size:(g + 1) * w.group_size] for (b, g) in groups])
+        s_g = torch.stack([stop[b, g:g + 1] for (b, g) in groups])
+        rep = compare(mini, o_g, s_g, art=art_on)
+        assert rep.stop_mismatch_nonfragile == 0, rep
+        assert rep.max_rel_err <= OUT_TOL[w.dtype], rep
+        # properties that hold at any size
+        assert (stop >= 0).all() and (loaded >= stop).all()
+        if not art_on:
+            _, s_ref, _ = run_oracle(mini, art=False)
+            assert np.array_equal(s_g.cpu().numpy(), s_ref)
+    del w
+    torch.cuda.empty_cache()
