@@ -11,8 +11,8 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 @pytest.fixture(scope="module")
 def art():
-    from paper_2606_00024_b200 import build
-    build.build()
+    import runpy                      # by path: the package refuses to import until the library exists
+    runpy.run_path(os.path.join(ROOT, "paper_2606_00024_b200", "build.py"))["build"]()
     import paper_2606_00024_b200 as a
     return a
 
