@@ -17,7 +17,8 @@ FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=s
 def needs_build() -> bool:
     if not os.path.exists(LIB):
         return True
-    deps = SRC + [os.path.join(ROOT, "include", "art_decode.h")]
+    csrc = os.path.join(HERE, "csrc")
+    deps = [os.path.join(csrc, f) for f in os.listdir(csrc)] + [os.path.join(ROOT, "include", "art_decode.h")]
     return any(os.path.getmtime(d) > os.path.getmtime(LIB) for d in deps)
 
 

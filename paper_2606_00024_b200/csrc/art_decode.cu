@@ -1,813 +1,113 @@
-// ART decode attention for B200 (sm_100a): kernels + C ABI (include/art_decode.h).
+// ART decode attention for B200 (sm_100a): host side and C ABI (include/art_decode.h).
 //
-// One thread-block CLUSTER of C CTAs per query group (sequence b, KV head g).  Traversal
-// steps t = 1..T are dealt round-robin: CTA c owns steps c+1, c+1+C, ...
-// Each CTA streams its blocks HBM -> shared memory with cp.async.bulk (TMA) into an
-// mbarrier ring, and its 8 compute warps each run an independent online-softmax stream over
-// 8 of the block's 64 tokens, keeping the block-local P~V_t SEPARATE
-// ("pending") until the termination decision for the preceding steps is known.  Every step's
-// summary (block max, block sum, the probe components of P~V_t; 2+m floats per head) goes
-// through distributed shared memory to the cluster leader, whose scan warp replays the
-// SEQUENTIAL criterion of Algorithm 1 (Eq. 2-3) in the recurrence form of
-// PAPER.md:320/361 and broadcasts progress / the stop step t*.  Blocks with step > t* are
-// discarded, so the result equals the sequential algorithm's for any C; the only cost is a
-// bounded number of prefetched-then-discarded blocks, which are counted in blocks_loaded.
-//
+// Two kernels sit behind the ABI, both walking the eligible KV blocks in the paper's order with the
+// exact sequential termination semantics of Algorithm 1:
+//   art_decode_tc.cuh    bf16 KV, head_dim 128: TMA tensor loads, tcgen05.mma with TMEM accumulators
+//   art_decode_simt.cuh  fp32 KV, head_dim 64:  TMA bulk loads, CUDA-core FMAs (1e-5 tolerance rules out TF32)
 // The ART-off entry point is the same kernel template with the detector compiled out.
-#include <cuda_runtime.h>
-#include <cuda_bf16.h>
-#include <stdint.h>
-#include <math.h>
-#include <type_traits>
-
-#include "art_decode.h"
+#include "art_decode_simt.cuh"
+#include "art_decode_tc.cuh"
 
 namespace art {
-
-constexpr int kBlockTokens = 64;
-constexpr int kRowBytes = 256;                    // one token row of one head: d * sizeof(T)
-constexpr int kTileBytes = kBlockTokens * kRowBytes;   // 16 KiB: K or V tile of one block
-constexpr int kStageBytes = 2 * kTileBytes;       // K + V
-constexpr int kComputeWarps = 8;
-constexpr int kProducerWarp = 8;
-constexpr int kScanWarp = 9;                      // summaries + (leader) the sequential criterion
-constexpr int kThreads = 320;
-constexpr int kMaxSmem = 232448;                  // 227 KiB usable per CTA on sm_100
-constexpr float kNegInf = -INFINITY;
-
-struct Params {
-  const void* q;
-  const uint8_t* k;
-  const uint8_t* v;
-  const int32_t* block_table;
-  const int32_t* elig;
-  const int32_t* elig_counts;
-  const int32_t* seq_lens;
-  float* out;
-  int32_t* stop_block;
-  int32_t* blocks_loaded;
-  int32_t batch, Hq, Hkv;
-  int32_t max_blocks, max_elig;
-  int32_t policy, layout, sink, window;
-  int64_t page_stride, head_stride, token_stride;   // bytes
-  float scale_log2;                                  // sm_scale * log2(e)
-  float tau, phi;
-  int32_t patience;
-  int32_t stages, mbox_slots;
-};
-
-// ----------------------------------------------------------------------------- PTX wrappers
-
-__device__ __forceinline__ uint32_t smem_u32(const void* p) {
-  return static_cast<uint32_t>(__cvta_generic_to_shared(p));
-}
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r;
-}
-__device__ __forceinline__ uint32_t cluster_nctarank() {
-  uint32_t r; asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r)); return r;
-}
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {
-  uint32_t r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank)); return r;
-}
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
-  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" :: "r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" :: "r"(bar) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
-  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_remote(uint32_t cluster_bar) {
-  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" :: "r"(cluster_bar) : "memory");
-}
-__device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile("{\n\t.reg .pred p;\n\t"
-               "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-               "selp.u32 %0, 1, 0, p;\n\t}"
-               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-  return ok != 0;
-}
-__device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
-  uint32_t ok;
-  asm volatile("{\n\t.reg .pred p;\n\t"
-               "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
-               "selp.u32 %0, 1, 0, p;\n\t}"
-               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
-  return ok != 0;
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  while (!mbar_try_wait(bar, parity)) {}
-}
-__device__ __forceinline__ void fence_mbar_init() {
-  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-}
-// TMA 1-D bulk copy global -> this CTA's shared memory, completion on an mbarrier.
-__device__ __forceinline__ void tma_load_1d(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
-  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-               :: "r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
-__device__ __forceinline__ void st_cluster_f32(uint32_t cluster_addr, float v) {
-  asm volatile("st.shared::cluster.f32 [%0], %1;" :: "r"(cluster_addr), "f"(v) : "memory");
-}
-__device__ __forceinline__ void st_cluster_release_s32(uint32_t cluster_addr, int v) {
-  asm volatile("st.release.cluster.shared::cluster.s32 [%0], %1;" :: "r"(cluster_addr), "r"(v) : "memory");
-}
-__device__ __forceinline__ float ld_cluster_f32(uint32_t cluster_addr) {
-  float v; asm volatile("ld.shared::cluster.f32 %0, [%1];" : "=f"(v) : "r"(cluster_addr) : "memory"); return v;
-}
-__device__ __forceinline__ int ld_cluster_s32(uint32_t cluster_addr) {
-  int v; asm volatile("ld.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(cluster_addr) : "memory"); return v;
-}
-__device__ __forceinline__ int ld_acquire_ctrl(uint32_t addr) {
-  int v; asm volatile("ld.acquire.cluster.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
-}
-__device__ __forceinline__ int ld_volatile_s32(uint32_t addr) {
-  int v; asm volatile("ld.volatile.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
-}
-__device__ __forceinline__ void st_volatile_s32(uint32_t addr, int v) {
-  asm volatile("st.volatile.shared::cta.s32 [%0], %1;" :: "r"(addr), "r"(v) : "memory");
-}
-__device__ __forceinline__ uint4 lds128(uint32_t addr) {
-  uint4 r; asm volatile("ld.shared.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "r"(addr));
-  return r;
-}
-__device__ __forceinline__ uint2 lds64(uint32_t addr) {
-  uint2 r; asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(addr));
-  return r;
-}
-__device__ __forceinline__ float fast_exp2(float x) {       // ex2.approx: exp2(-inf) = +0
-  float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y;
-}
-
-// ----------------------------------------------------------------------------- element types
-
-template <typename T> struct Elem;
-template <> struct Elem<float> {
-  static constexpr int E16 = 4, E8 = 2;
-  static __device__ __forceinline__ void cvt16(const uint4& r, float (&f)[4]) {
-    f[0] = __uint_as_float(r.x); f[1] = __uint_as_float(r.y); f[2] = __uint_as_float(r.z); f[3] = __uint_as_float(r.w);
-  }
-  static __device__ __forceinline__ void cvt8(const uint2& r, float (&f)[2]) {
-    f[0] = __uint_as_float(r.x); f[1] = __uint_as_float(r.y);
-  }
-};
-template <> struct Elem<__nv_bfloat16> {
-  static constexpr int E16 = 8, E8 = 4;
-  static __device__ __forceinline__ void cvt16(const uint4& r, float (&f)[8]) {
-    f[0] = __uint_as_float(r.x << 16); f[1] = __uint_as_float(r.x & 0xffff0000u);
-    f[2] = __uint_as_float(r.y << 16); f[3] = __uint_as_float(r.y & 0xffff0000u);
-    f[4] = __uint_as_float(r.z << 16); f[5] = __uint_as_float(r.z & 0xffff0000u);
-    f[6] = __uint_as_float(r.w << 16); f[7] = __uint_as_float(r.w & 0xffff0000u);
-  }
-  static __device__ __forceinline__ void cvt8(const uint2& r, float (&f)[4]) {
-    f[0] = __uint_as_float(r.x << 16); f[1] = __uint_as_float(r.x & 0xffff0000u);
-    f[2] = __uint_as_float(r.y << 16); f[3] = __uint_as_float(r.y & 0xffff0000u);
-  }
-};
-__device__ __forceinline__ float to_float(float x) { return x; }
-__device__ __forceinline__ float to_float(__nv_bfloat16 x) { return __bfloat162float(x); }
-
-// ----------------------------------------------------------------------------- traversal (A1)
-
-// Traversal order of the eligible blocks (SINK_WINDOW per reading R3).
-struct Trav {
-  int T;        // number of steps
-  int nb;       // blocks holding tokens < L
-  int sb;       // blocks holding sink tokens
-  int wb;       // first block holding window tokens (== nb if none)
-  int policy;
-  const int32_t* list;
-};
-
-__device__ __forceinline__ Trav make_trav(const Params& p, int b, int g, int L) {
-  Trav tr;
-  tr.policy = p.policy; tr.list = nullptr;
-  tr.nb = (L + kBlockTokens - 1) / kBlockTokens; tr.sb = 0; tr.wb = tr.nb;
-  if (p.policy == ART_POLICY_LIST) {
-    tr.list = p.elig + (static_cast<int64_t>(b) * p.Hkv + g) * p.max_elig;
-    tr.T = p.elig_counts[b * p.Hkv + g];
-  } else if (p.policy == ART_POLICY_SINK_WINDOW) {
-    const int s_eff = min(max(p.sink, 0), L);
-    tr.sb = (s_eff + kBlockTokens - 1) / kBlockTokens;
-    const int w0 = L - min(max(p.window, 0), L);           // first window token
-    tr.wb = (w0 < L) ? w0 / kBlockTokens : tr.nb;
-    if (tr.sb > 0) tr.T = (tr.wb <= tr.sb) ? tr.nb : 1 + (tr.nb - tr.wb) + (tr.sb - 1);
-    else tr.T = tr.nb - tr.wb;
-  } else {
-    tr.T = tr.nb;
-  }
-  if (L <= 0 && p.policy != ART_POLICY_LIST) tr.T = 0;
-  return tr;
-}
-
-// logical block id visited at 1-based step t
-__device__ __forceinline__ int trav_block(const Trav& tr, int t) {
-  if (tr.policy == ART_POLICY_LIST) return tr.list[t - 1];
-  if (tr.policy == ART_POLICY_SINK_WINDOW && tr.sb > 0) {
-    if (t == 1) return 0;                                   // the sink block is never skipped (R3)
-    const int k = t - 2;
-    if (tr.wb <= tr.sb) return tr.nb - 1 - k;
-    const int n1 = tr.nb - tr.wb;
-    return (k < n1) ? tr.nb - 1 - k : tr.sb - 1 - (k - n1);
-  }
-  return (tr.policy == ART_POLICY_SINK_WINDOW ? tr.nb : tr.T) - t;   // most recent first
-}
-
-__device__ __forceinline__ uint64_t range_mask(int lo, int hi) {     // bits [lo, hi) of 64
-  lo = max(lo, 0); hi = min(hi, 64);
-  if (hi <= lo) return 0ull;
-  const uint64_t upper = (hi >= 64) ? ~0ull : ((1ull << hi) - 1ull);
-  return upper & ~((1ull << lo) - 1ull);
-}
-
-// which of the block's 64 tokens are eligible (partial last block, sink / window edges; R8)
-__device__ __forceinline__ uint64_t block_mask(const Params& p, int L, int blk) {
-  if (blk < 0) return 0ull;
-  const int64_t j0 = static_cast<int64_t>(blk) * kBlockTokens;
-  if (j0 >= L) return 0ull;
-  const int base = static_cast<int>(j0);
-  if (p.policy == ART_POLICY_SINK_WINDOW) {
-    const int s_eff = min(max(p.sink, 0), L);
-    const int w0 = L - min(max(p.window, 0), L);
-    return range_mask(0, s_eff - base) | range_mask(w0 - base, L - base);
-  }
-  return range_mask(0, L - base);
-}
-
-// ----------------------------------------------------------------------------- warp helpers
-
-// Sum N values over the 16 lanes of a half-warp with a transposing butterfly: while more than
-// one value is left each step halves the value count; afterwards lane l holds, in v[0], the
-// full sum of value head_of_lane(l).
-template <int N, int MASK>
-struct Reduce16 {
-  static __device__ __forceinline__ void run(float* v, int lane) {
-    if constexpr (N > 1) {
-      constexpr int n = N / 2;
-      const bool up = (lane & MASK) != 0;
-#pragma unroll
-      for (int i = 0; i < n; ++i) {
-        const float keep = up ? v[i + n] : v[i];
-        const float send = up ? v[i] : v[i + n];
-        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, MASK);
-      }
-      if constexpr (MASK > 1) Reduce16<n, MASK / 2>::run(v, lane);
-    } else {
-      v[0] += __shfl_xor_sync(0xffffffffu, v[0], MASK);
-      if constexpr (MASK > 1) Reduce16<1, MASK / 2>::run(v, lane);
-    }
-  }
-};
-
-template <int G> __device__ __forceinline__ int head_of_lane(int lane) {   // which value Reduce16 leaves in this lane
-  int h = 0;
-  if constexpr (G >= 2) h += ((lane >> 3) & 1) * (G / 2);
-  if constexpr (G >= 4) h += ((lane >> 2) & 1) * (G / 4);
-  if constexpr (G >= 8) h += ((lane >> 1) & 1) * (G / 8);
-  return h;
-}
-template <int G> __device__ __forceinline__ constexpr int lane_of_head(int h) {   // first lane (0..15) holding head h
-  int l = 0;
-  if constexpr (G >= 2) l |= ((h / (G / 2)) & 1) << 3;
-  if constexpr (G >= 4) l |= ((h / (G / 4)) & 1) << 2;
-  if constexpr (G >= 8) l |= ((h / (G / 8)) & 1) << 1;
-  return l;
-}
-
-// ----------------------------------------------------------------------------- shared memory map
-
-struct StageInfo { unsigned long long mask; int blk; int pad; };
-
-struct SmemMap {
-  uint32_t ring, sumbuf, mbox, info, bars, misc, total;
-  // barrier indices inside `bars` (8 bytes each)
-  uint32_t full0, empty0, sumready0, sumfree0, mbox0;
-};
-
-__host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int mslots, bool art) {
-  SmemMap m;
-  uint32_t off = 0;
-  m.ring = off; off += static_cast<uint32_t>(stages) * kStageBytes;
-  const uint32_t row = static_cast<uint32_t>(G) * (2 + PW) * 4;
-  m.sumbuf = off; off += art ? 2u * kComputeWarps * row : 0u;
-  m.mbox = off; off += art ? static_cast<uint32_t>(mslots) * row : 0u;
-  off = (off + 15u) & ~15u;
-  m.info = off; off += static_cast<uint32_t>(stages) * 16u;
-  m.bars = off;
-  m.full0 = 0; m.empty0 = stages; m.sumready0 = 2 * stages; m.sumfree0 = 2 * stages + 2; m.mbox0 = 2 * stages + 4;
-  off += (2u * stages + 4u + (art ? mslots : 0)) * 8u;
-  m.misc = off; off += 64u + 16u * 4u;   // ctrl, n_issued, loaded, cta_m[8], cta_l[8]
-  m.total = (off + 127u) & ~127u;
-  return m;
-}
-
-// misc words
-constexpr uint32_t kCtrl = 0, kIssued = 4, kLoaded = 8, kCtaM = 64, kCtaL = 96;
-
-// ----------------------------------------------------------------------------- the kernel
-
-// MODE 0: ART off.  MODE 1: ART on, probe = 32 coordinates k*(d/32).  MODE 2: ART on, probe = all d.
-template <typename T, int D, int G, int MODE>
-__global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p) {
-  constexpr bool ART = MODE != 0;
-  constexpr int PW = (MODE == 2) ? D : 32;           // probe width m
-  constexpr int E16 = Elem<T>::E16, E8 = Elem<T>::E8;
-  constexpr int ROWF = 2 + PW;                       // summary floats per head: max, sum, probe
-  static_assert(D * sizeof(T) == kRowBytes, "token row must be 256 bytes");
-  static_assert(D / 32 == E8, "one probe coordinate per 8-byte chunk");
-
-  extern __shared__ __align__(128) uint8_t smem[];
-  const int S = p.stages, M = p.mbox_slots;
-  const SmemMap sm = make_smem_map(G, PW, S, M, ART);
-  const uint32_t sbase = smem_u32(smem);
-  const uint32_t bars = sbase + sm.bars;
-  auto bar = [&](uint32_t idx) { return bars + idx * 8u; };
-  const uint32_t a_ctrl = sbase + sm.misc + kCtrl, a_issued = sbase + sm.misc + kIssued,
-                 a_loaded = sbase + sm.misc + kLoaded;
-  float* sumbuf = reinterpret_cast<float*>(smem + sm.sumbuf);
-  float* mbox = reinterpret_cast<float*>(smem + sm.mbox);
-  StageInfo* info = reinterpret_cast<StageInfo*>(smem + sm.info);
-
-  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int C = static_cast<int>(cluster_nctarank());
-  const int rank = static_cast<int>(cluster_ctarank());
-  const int group = blockIdx.x / C;
-  const int b = group / p.Hkv, g = group % p.Hkv;
-  const int L = p.seq_lens[b];
-  const Trav tr = make_trav(p, b, g, L);
-  const int Tn = tr.T;
-  const int n_c = (Tn > rank) ? (Tn - rank + C - 1) / C : 0;   // steps owned by this CTA
-
-  if (tid == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), kComputeWarps); }
-    mbar_init(bar(sm.sumready0), kComputeWarps); mbar_init(bar(sm.sumready0 + 1), kComputeWarps);
-    mbar_init(bar(sm.sumfree0), 1); mbar_init(bar(sm.sumfree0 + 1), 1);
-    if (ART) for (int s = 0; s < M; ++s) mbar_init(bar(sm.mbox0 + s), 32);
-    st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_issued, 0x7fffffff); st_volatile_s32(a_loaded, 0);
-    fence_mbar_init();
-  }
-  cluster_sync_all();   // barriers of every CTA of the cluster are live before any remote arrive
-
-  // per-warp flash state (compute warps); declared here so the epilogue can see it
-  float acc[G][E8], m_w[G], l_w[G];
-#pragma unroll
-  for (int h = 0; h < G; ++h) {
-    m_w[h] = kNegInf; l_w[h] = 0.f;
-#pragma unroll
-    for (int e = 0; e < E8; ++e) acc[h][e] = 0.f;
-  }
-
-  // "fired and step t lies beyond t*": every wait that could otherwise hang forever checks this
-  auto beyond_stop = [&](int t) -> bool {
-    if constexpr (!ART) return false;
-    const int c = ld_acquire_ctrl(a_ctrl);
-    return c < 0 && t > -c;
-  };
-
-  if (warp == kProducerWarp) {
-    // ===================================================== A1 + A2: resolve blocks, issue TMA loads
-    int it_issued = 0, loaded = 0;
-    bool stop = false;
-    for (int i0 = 0; i0 < n_c && !stop; i0 += 32) {
-      const int i = i0 + lane;
-      int blk = -1; unsigned long long mask = 0ull; long long off = 0;
-      if (i < n_c) {
-        blk = trav_block(tr, i * C + rank + 1);
-        mask = block_mask(p, L, blk);
-        if (mask) {
-          const int page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
-          off = static_cast<int64_t>(page) * p.page_stride + static_cast<int64_t>(g) * p.head_stride;
-        }
-      }
-      const int cnt = min(32, n_c - i0);
-      for (int kk = 0; kk < cnt; ++kk) {
-        const int it = i0 + kk, stage = it % S, t = it * C + rank + 1;
-        const int blk_k = __shfl_sync(0xffffffffu, blk, kk);
-        const unsigned long long mask_k = __shfl_sync(0xffffffffu, mask, kk);
-        const long long off_k = __shfl_sync(0xffffffffu, off, kk);
-        if (it >= S) {                                       // slot must have been released
-          const uint32_t par = ((it / S) - 1) & 1;
-          while (!mbar_try_wait(bar(sm.empty0 + stage), par)) { if (beyond_stop(t)) { stop = true; break; } }
-        }
-        if (!stop && beyond_stop(t)) stop = true;            // A7: stop issuing prefetch once fired
-        if (stop) break;
-        const uint32_t fb = bar(sm.full0 + stage);
-        const uint32_t dstK = sbase + sm.ring + stage * kStageBytes, dstV = dstK + kTileBytes;
-        if (lane == 0) { info[stage].mask = mask_k; info[stage].blk = blk_k; }
-        if (mask_k == 0ull) {
-          if (lane == 0) mbar_arrive(fb);                    // nothing to load: an all-masked step
-        } else if (p.layout == ART_LAYOUT_HND) {
-          if (lane == 0) {
-            mbar_arrive_expect_tx(fb, kStageBytes);
-            tma_load_1d(dstK, p.k + off_k, kTileBytes, fb);
-            tma_load_1d(dstV, p.v + off_k, kTileBytes, fb);
-          }
-          ++loaded;
-        } else {                                             // NHD: one 256-byte row per (token)
-          if (lane == 0) mbar_arrive_expect_tx(fb, kStageBytes);
-          __syncwarp();
-#pragma unroll
-          for (int rr = 0; rr < 2; ++rr) {
-            const int r = lane * 2 + rr;
-            tma_load_1d(dstK + r * kRowBytes, p.k + off_k + r * p.token_stride, kRowBytes, fb);
-            tma_load_1d(dstV + r * kRowBytes, p.v + off_k + r * p.token_stride, kRowBytes, fb);
-          }
-          ++loaded;
-        }
-        it_issued = it + 1;
-      }
-    }
-    if (lane == 0) { st_volatile_s32(a_issued, it_issued); st_volatile_s32(a_loaded, loaded); }
-    // drain: bulk copies still in flight must land before the CTA reuses the ring or exits (H5)
-    for (int j = max(0, it_issued - S); j < it_issued; ++j) mbar_wait(bar(sm.full0 + j % S), (j / S) & 1);
-  } else if (warp < kComputeWarps) {
-    // ===================================================== A3-A5: scores, online softmax, P.V
-    const int half = lane >> 4, c16 = lane & 15;
-    float qreg[G][E16];                                      // this lane's 16-byte chunk of every head's q
-    {
-      const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * G) * D + c16 * E16;
-#pragma unroll
-      for (int h = 0; h < G; ++h)
-#pragma unroll
-        for (int e = 0; e < E16; ++e) qreg[h][e] = to_float(qp[h * D + e]) * p.scale_log2;
-    }
-    float pend[G][E8], pend_m[G], pend_l[G];
-    bool have_pend = false; int pend_t = 0;
-#pragma unroll
-    for (int h = 0; h < G; ++h) { pend_m[h] = kNegInf; pend_l[h] = 0.f;
-#pragma unroll
-      for (int e = 0; e < E8; ++e) pend[h][e] = 0.f; }
-
-    auto fold = [&](const float (&val)[G][E8], const float (&mt)[G], const float (&lt)[G]) {
-#pragma unroll
-      for (int h = 0; h < G; ++h) {
-        const float mn = fmaxf(m_w[h], mt[h]);
-        if (mn == kNegInf) continue;
-        const float a = fast_exp2(m_w[h] - mn), bb = fast_exp2(mt[h] - mn);
-        l_w[h] = a * l_w[h] + bb * lt[h];
-#pragma unroll
-        for (int e = 0; e < E8; ++e) acc[h][e] = a * acc[h][e] + bb * val[h][e];
-        m_w[h] = mn;
-      }
-    };
-    auto wait_decision = [&](int need) -> int {              // progress >= need, or fired
-      int c;
-      do { c = ld_acquire_ctrl(a_ctrl); } while (c >= 0 && c < need);
-      return c;
-    };
-
-    for (int i = 0; i < n_c; ++i) {
-      const int stage = i % S, t = i * C + rank + 1;
-      {
-        bool got = false;
-        const uint32_t par = (i / S) & 1;
-        while (true) {
-          if (mbar_try_wait(bar(sm.full0 + stage), par)) { got = true; break; }
-          if (ART && ld_volatile_s32(a_issued) <= i) break;   // the producer stopped before this step
-        }
-        if (!got) break;
-      }
-      const unsigned long long vmask = info[stage].mask;
-      const uint32_t Kt = sbase + sm.ring + stage * kStageBytes, Vt = Kt + kTileBytes;
-
-      // ---- A3: s = q.k / sqrt(d) (log2 domain) for this warp's 8 tokens; lane ends with head hl
-      float sv[4];
-#pragma unroll
-      for (int pp = 0; pp < 4; ++pp) {
-        const int r = warp * 8 + pp * 2 + half;
-        float kv[E16];
-        Elem<T>::cvt16(lds128(Kt + r * kRowBytes + c16 * 16), kv);
-        float s[G];
-#pragma unroll
-        for (int h = 0; h < G; ++h) {
-          float a = 0.f;
-#pragma unroll
-          for (int e = 0; e < E16; ++e) a = fmaf(qreg[h][e], kv[e], a);
-          s[h] = a;
-        }
-        Reduce16<G, 8>::run(s, lane);
-        sv[pp] = ((vmask >> r) & 1ull) ? s[0] : kNegInf;     // masked tokens: weight 0 (R8)
-      }
-      // ---- A4: block-local softmax over the warp's 8 tokens
-      float mloc = fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[2], sv[3]));
-      mloc = fmaxf(mloc, __shfl_xor_sync(0xffffffffu, mloc, 16));
-      float pr[4], lsum = 0.f;
-#pragma unroll
-      for (int pp = 0; pp < 4; ++pp) { pr[pp] = (sv[pp] == kNegInf) ? 0.f : fast_exp2(sv[pp] - mloc); lsum += pr[pp]; }
-      lsum += __shfl_xor_sync(0xffffffffu, lsum, 16);
-      float mt[G], lt[G];
-#pragma unroll
-      for (int h = 0; h < G; ++h) {
-        mt[h] = __shfl_sync(0xffffffffu, mloc, lane_of_head<G>(h));
-        lt[h] = __shfl_sync(0xffffffffu, lsum, lane_of_head<G>(h));
-      }
-      // ---- A5: P~V for the warp's 8 tokens; lane owns the 8-byte chunk `lane` of every row
-      float nw[G][E8];
-#pragma unroll
-      for (int h = 0; h < G; ++h)
-#pragma unroll
-        for (int e = 0; e < E8; ++e) nw[h][e] = 0.f;
-#pragma unroll
-      for (int rr = 0; rr < 8; ++rr) {
-        const int r = warp * 8 + rr;
-        float ph[G];
-#pragma unroll
-        for (int h = 0; h < G; ++h) ph[h] = __shfl_sync(0xffffffffu, pr[rr >> 1], (rr & 1) * 16 + lane_of_head<G>(h));
-        if ((vmask >> r) & 1ull) {                           // warp-uniform; masked rows may hold NaN
-          float vv[E8];
-          Elem<T>::cvt8(lds64(Vt + r * kRowBytes + lane * 8), vv);
-#pragma unroll
-          for (int h = 0; h < G; ++h)
-#pragma unroll
-            for (int e = 0; e < E8; ++e) nw[h][e] = fmaf(ph[h], vv[e], nw[h][e]);
-        }
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.empty0 + stage));    // K/V tile consumed: slot free
-
-      if constexpr (!ART) {
-        fold(nw, mt, lt);
-      } else {
-        // ---- publish this warp's share of the step summary (max, sum, probe part of P~V)
-        const int par = i & 1;
-        bool discard = false;
-        if (i >= 2) {
-          const uint32_t ph2 = ((i >> 1) - 1) & 1;
-          while (!mbar_try_wait(bar(sm.sumfree0 + par), ph2)) { if (beyond_stop(t)) { discard = true; break; } }
-        }
-        if (discard) break;                                  // t > t*: this block is not part of the result
-        float* sb = sumbuf + static_cast<size_t>(par * kComputeWarps + warp) * G * ROWF;
-#pragma unroll
-        for (int h = 0; h < G; ++h) {
-          if constexpr (MODE == 1) sb[h * ROWF + 2 + lane] = nw[h][0];      // coordinate lane*(d/32)  (R1)
-          else {
-#pragma unroll
-            for (int e = 0; e < E8; ++e) sb[h * ROWF + 2 + lane * E8 + e] = nw[h][e];
-          }
-          if (lane == h) { sb[h * ROWF] = mt[h]; sb[h * ROWF + 1] = lt[h]; }
-        }
-        __syncwarp();
-        if (lane == 0) mbar_arrive(bar(sm.sumready0 + par));
-        // ---- fold the PREVIOUS block once the decision for everything before it is known
-        if (have_pend) {
-          const int c = wait_decision(pend_t - 1);
-          have_pend = false;
-          if (c < 0 && pend_t > -c) break;                   // previous (and so this) block lies beyond t*
-          fold(pend, pend_m, pend_l);
-          if (c < 0 && t > -c) break;
-        }
-#pragma unroll
-        for (int h = 0; h < G; ++h) { pend_m[h] = mt[h]; pend_l[h] = lt[h];
-#pragma unroll
-          for (int e = 0; e < E8; ++e) pend[h][e] = nw[h][e]; }
-        have_pend = true; pend_t = t;
-      }
-    }
-    if (ART && have_pend) {
-      const int c = wait_decision(pend_t - 1);
-      if (!(c < 0 && pend_t > -c)) fold(pend, pend_m, pend_l);
-    }
-  } else if (ART && warp == kScanWarp) {
-    // ===================================================== A6 + A7 + A9: summaries, sequential criterion
-    constexpr int LPH = 32 / G;                              // lanes per head
-    constexpr int CPL = PW / LPH;                            // probe components per lane
-    const int h = lane / LPH, sub = lane % LPH;
-
-    // merge the 8 warps' shares of local iteration i into one step summary (mt, lt, pv[])
-    auto merge_local = [&](int i, int t, float& mt, float& lt, float (&pv)[CPL]) -> bool {
-      const int par = i & 1;
-      const uint32_t ph = (i >> 1) & 1;
-      while (!mbar_try_wait(bar(sm.sumready0 + par), ph)) { if (beyond_stop(t)) return false; }
-      const float* sb = sumbuf + static_cast<size_t>(par * kComputeWarps) * G * ROWF + h * ROWF;
-      float mw[kComputeWarps];
-      mt = kNegInf;
-#pragma unroll
-      for (int w = 0; w < kComputeWarps; ++w) { mw[w] = sb[w * G * ROWF]; mt = fmaxf(mt, mw[w]); }
-      lt = 0.f;
-#pragma unroll
-      for (int j = 0; j < CPL; ++j) pv[j] = 0.f;
-#pragma unroll
-      for (int w = 0; w < kComputeWarps; ++w) {
-        const float f = (mw[w] == kNegInf) ? 0.f : fast_exp2(mw[w] - mt);
-        lt = fmaf(f, sb[w * G * ROWF + 1], lt);
-#pragma unroll
-        for (int j = 0; j < CPL; ++j) pv[j] = fmaf(f, sb[w * G * ROWF + 2 + sub + LPH * j], pv[j]);
-      }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.sumfree0 + par));
-      return true;
-    };
-
-    if (rank == 0) {
-      // ---- leader: Algorithm 1's loop over steps, on summaries
-      float m_run = kNegInf, l_run = 0.f, x[CPL];
-#pragma unroll
-      for (int j = 0; j < CPL; ++j) x[j] = 0.f;              // x^(0) = 0 (Alg. 1 l.1)
-      int cnt = 0, t_stop = 0;                               // c^(0) = 0 (l.2)
-      uint32_t phasebits = 0;
-      for (int t = 1; t <= Tn; ++t) {
-        const int owner = (t - 1) % C;
-        float mt, lt, pv[CPL];
-        if (owner == 0) {
-          merge_local((t - 1) / C, t, mt, lt, pv);
-        } else {
-          const int slot = (t - 1) % M;
-          while (!mbar_try_wait_cluster(bar(sm.mbox0 + slot), (phasebits >> slot) & 1u)) {}
-          phasebits ^= 1u << slot;
-          const float* mb = mbox + static_cast<size_t>(slot) * G * ROWF + h * ROWF;
-          mt = mb[0]; lt = mb[1];
-#pragma unroll
-          for (int j = 0; j < CPL; ++j) pv[j] = mb[2 + sub + LPH * j];
-        }
-        // streaming update in recurrence form: x^(t) - x^(t-1) = (l_t / A_t) P(u^(t) - o^(t-1))
-        // (PAPER.md:320, :361), with l_t u^(t) = P~V_t and everything relative to the running max.
-        float sdd = 0.f, sad = 0.f, saa = 0.f, sbb = 0.f;
-        if (mt != kNegInf) {                                 // a step with no valid token changes nothing (R8)
-          const float mn = fmaxf(m_run, mt);
-          const float al = fast_exp2(m_run - mn), be = fast_exp2(mt - mn);
-          const float l_new = fmaf(al, l_run, be * lt);
-          const float r = be / l_new;
-#pragma unroll
-          for (int j = 0; j < CPL; ++j) {
-            const float dlt = r * fmaf(-lt, x[j], pv[j]);
-            const float xn = x[j] + dlt;
-            sdd = fmaf(dlt, dlt, sdd); sad = fmaf(x[j], dlt, sad); saa = fmaf(x[j], x[j], saa); sbb = fmaf(xn, xn, sbb);
-            x[j] = xn;
-          }
-          m_run = mn; l_run = l_new;
-        } else {
-#pragma unroll
-          for (int j = 0; j < CPL; ++j) { saa = fmaf(x[j], x[j], saa); }
-          sbb = saa;
-        }
-#pragma unroll
-        for (int msk = LPH / 2; msk >= 1; msk >>= 1) {
-          sdd += __shfl_xor_sync(0xffffffffu, sdd, msk); sad += __shfl_xor_sync(0xffffffffu, sad, msk);
-          saa += __shfl_xor_sync(0xffffffffu, saa, msk); sbb += __shfl_xor_sync(0xffffffffu, sbb, msk);
-        }
-        // Eq. 2: d_scale = ||dx||; d_direction = 1 - cos(x_new, x_old), evaluated as
-        // (|a|^2 |d|^2 - (a.d)^2) / (|a||b| (|a||b| + a.b)) to avoid the cancellation in 1 - cos.
-        const float d_scale = sqrtf(sdd);
-        float d_dir = 1.f;                                   // zero norm => cos := 0 (R4)
-        if (saa > 0.f && sbb > 0.f) {
-          const float nanb = sqrtf(saa) * sqrtf(sbb);
-          const float ab = saa + sad;
-          if (ab > 0.f) d_dir = fmaxf(fmaf(saa, sdd, -sad * sad), 0.f) / (nanb * (nanb + ab));
-          else d_dir = 1.f - ab / nanb;
-        }
-        const bool stable_h = (d_scale < p.tau) && (d_dir < p.phi);          // strict (R5)
-        const bool stable = __all_sync(0xffffffffu, stable_h);               // AND over the group's heads (R2)
-        cnt = stable ? cnt + 1 : 0;                                          // Eq. 3
-        const bool fire = cnt >= p.patience;
-        if (lane < C) st_cluster_release_s32(mapa(a_ctrl, lane), fire ? -t : t);
-        if (fire) { t_stop = t; break; }
-      }
-      if (lane == 0) p.stop_block[group] = t_stop ? t_stop : Tn;             // t* (R9)
-    } else {
-      // ---- other CTAs: ship each own step's summary to the leader's mailbox
-      for (int i = 0; i < n_c; ++i) {
-        const int t = i * C + rank + 1;
-        float mt, lt, pv[CPL];
-        if (!merge_local(i, t, mt, lt, pv)) break;
-        bool dead = false;                                   // the slot must have been consumed: step t - M scanned
-        while (true) {
-          const int c = ld_acquire_ctrl(a_ctrl);
-          if (c < 0) { dead = t > -c; break; }
-          if (c >= t - M) break;
-        }
-        if (dead) break;
-        const int slot = (t - 1) % M;
-        const uint32_t row = sbase + sm.mbox + (static_cast<uint32_t>(slot) * G + h) * ROWF * 4u;
-        const uint32_t rrow = mapa(row, 0);
-        if (sub == 0) { st_cluster_f32(rrow, mt); st_cluster_f32(rrow + 4, lt); }
-#pragma unroll
-        for (int j = 0; j < CPL; ++j) st_cluster_f32(rrow + (2 + sub + LPH * j) * 4u, pv[j]);
-        mbar_arrive_remote(mapa(bar(sm.mbox0 + slot), 0));   // release.cluster: this lane's stores first
-      }
-    }
-  }
-
-  // ===================================================== A8 / A9: combine partial states, write out
-  __syncthreads();                                           // ring is free: all loads drained, all warps done
-  float* part = reinterpret_cast<float*>(smem + sm.ring);    // [8][G][D] + pm[8][G] + pl[8][G] + cta[G][D]
-  float* pm = part + kComputeWarps * G * D;
-  float* pl = pm + kComputeWarps * G;
-  float* cta = pl + kComputeWarps * G;
-  if (warp < kComputeWarps) {
-#pragma unroll
-    for (int h = 0; h < G; ++h) {
-#pragma unroll
-      for (int e = 0; e < E8; ++e) part[(warp * G + h) * D + lane * E8 + e] = acc[h][e];
-      if (lane == h) { pm[warp * G + h] = m_w[h]; pl[warp * G + h] = l_w[h]; }
-    }
-  }
-  __syncthreads();
-  float* cta_m = reinterpret_cast<float*>(smem + sm.misc + kCtaM);
-  float* cta_l = reinterpret_cast<float*>(smem + sm.misc + kCtaL);
-  for (int o = tid; o < G * D; o += kThreads) {
-    const int h = o / D;
-    float mx = kNegInf;
-#pragma unroll
-    for (int w = 0; w < kComputeWarps; ++w) mx = fmaxf(mx, pm[w * G + h]);
-    float a = 0.f, l = 0.f;
-#pragma unroll
-    for (int w = 0; w < kComputeWarps; ++w) {
-      const float f = (pm[w * G + h] == kNegInf) ? 0.f : fast_exp2(pm[w * G + h] - mx);
-      a = fmaf(f, part[(w * G + h) * D + (o - h * D)], a);
-      l = fmaf(f, pl[w * G + h], l);
-    }
-    cta[o] = a;
-    if (o == h * D) { cta_m[h] = mx; cta_l[h] = l; }
-  }
-  cluster_sync_all();
-  if (rank == 0) {
-    for (int o = tid; o < G * D; o += kThreads) {
-      const int h = o / D;
-      float mx = kNegInf;
-      for (int c = 0; c < C; ++c) mx = fmaxf(mx, ld_cluster_f32(mapa(smem_u32(&cta_m[h]), c)));
-      float a = 0.f, l = 0.f;
-      for (int c = 0; c < C; ++c) {
-        const float mc = ld_cluster_f32(mapa(smem_u32(&cta_m[h]), c));
-        const float f = (mc == kNegInf) ? 0.f : fast_exp2(mc - mx);
-        a = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta[o]), c)), a);
-        l = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta_l[h]), c)), l);
-      }
-      p.out[(static_cast<int64_t>(b) * p.Hq + g * G) * D + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
-    }
-    if (tid == 0) {
-      if (!ART) p.stop_block[group] = Tn;
-      if (p.blocks_loaded) {
-        int tot = 0;
-        for (int c = 0; c < C; ++c) tot += ld_cluster_s32(mapa(a_loaded, c));
-        p.blocks_loaded[group] = tot;
-      }
-    }
-  }
-  cluster_sync_all();                                        // peers' shared memory stays alive until read
-}
 
 // ----------------------------------------------------------------------------- host side
 
 struct LaunchPlan { int C, stages, mslots; uint32_t smem; };
 
-template <typename T, int D, int G, int MODE>
-static cudaError_t launch_one(const Params& p, int groups, int C, uint32_t smem_bytes, cudaStream_t stream) {
-  auto kern = art_decode_kernel<T, D, G, MODE>;
+static void set_cluster_attr(cudaLaunchAttribute* attr, int C) {
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+}
+
+template <typename Kern>
+static cudaError_t prepare_kernel(Kern kern, int C, uint32_t smem_bytes) {
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes));
   if (e != cudaSuccess) return e;
-  if (C > 8) {
-    e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-    if (e != cudaSuccess) return e;
-  }
+  if (C > 8) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
+  return e;
+}
+
+template <typename Kern, typename... Args>
+static cudaError_t launch_cluster(Kern kern, int threads, int groups, int C, uint32_t smem_bytes, cudaStream_t stream,
+                                  Args... args) {
+  cudaError_t e = prepare_kernel(kern, C, smem_bytes);
+  if (e != cudaSuccess) return e;
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(static_cast<unsigned>(groups) * C, 1, 1);
-  cfg.blockDim = dim3(kThreads, 1, 1);
+  cfg.blockDim = dim3(threads, 1, 1);
   cfg.dynamicSmemBytes = smem_bytes;
   cfg.stream = stream;
   cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  set_cluster_attr(attr, C);
   cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kern, p);
+  return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <typename T, int D, int G, int MODE>
-static int max_active_clusters(int C, uint32_t smem_bytes) {
-  auto kern = art_decode_kernel<T, D, G, MODE>;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes)) != cudaSuccess) return 0;
-  if (C > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return 0;
+template <typename Kern>
+static int max_active_clusters(Kern kern, int threads, int C, uint32_t smem_bytes) {
+  if (prepare_kernel(kern, C, smem_bytes) != cudaSuccess) { cudaGetLastError(); return 0; }
   cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(C, 1, 1); cfg.blockDim = dim3(kThreads, 1, 1); cfg.dynamicSmemBytes = smem_bytes;
+  cfg.gridDim = dim3(C, 1, 1); cfg.blockDim = dim3(threads, 1, 1); cfg.dynamicSmemBytes = smem_bytes;
   cudaLaunchAttribute attr[1];
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  set_cluster_attr(attr, C);
   cfg.attrs = attr; cfg.numAttrs = 1;
   int n = 0;
   if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
   return n;
 }
 
-// dispatch over (dtype/head_dim, G, MODE) with a generic functor
+// dispatch over (G, MODE) with a generic functor f(mode_constant, G_constant)
 template <typename F>
-static int dispatch(int dtype, int D, int G, int mode, F&& f) {
-#define ART_CASE_G(TT, DD, GG)                                                              \
-  if (G == GG) {                                                                              \
-    if (mode == 0) return f(std::integral_constant<int, 0>{}, TT{}, std::integral_constant<int, DD>{}, std::integral_constant<int, GG>{}); \
-    if (mode == 1) return f(std::integral_constant<int, 1>{}, TT{}, std::integral_constant<int, DD>{}, std::integral_constant<int, GG>{}); \
-    return f(std::integral_constant<int, 2>{}, TT{}, std::integral_constant<int, DD>{}, std::integral_constant<int, GG>{});                 \
+static int dispatch(int G, int mode, F&& f) {
+#define ART_CASE_G(GG)                                                                                   \
+  if (G == GG) {                                                                                         \
+    if (mode == 0) return f(std::integral_constant<int, 0>{}, std::integral_constant<int, GG>{});        \
+    if (mode == 1) return f(std::integral_constant<int, 1>{}, std::integral_constant<int, GG>{});        \
+    return f(std::integral_constant<int, 2>{}, std::integral_constant<int, GG>{});                       \
   }
-#define ART_CASE_T(TT, DD) { ART_CASE_G(TT, DD, 1) ART_CASE_G(TT, DD, 2) ART_CASE_G(TT, DD, 4) ART_CASE_G(TT, DD, 8) }
-  if (dtype == ART_DTYPE_F32 && D == 64) ART_CASE_T(float, 64)
-  if (dtype == ART_DTYPE_BF16 && D == 128) ART_CASE_T(__nv_bfloat16, 128)
-#undef ART_CASE_T
+  ART_CASE_G(1) ART_CASE_G(2) ART_CASE_G(4) ART_CASE_G(8)
 #undef ART_CASE_G
-  return ART_ERR_DTYPE;
+  return ART_ERR_SHAPE;
+}
+
+// ---- TMA tensor maps over the paged caches (bf16 path).  cuTensorMapEncodeTiled is a driver entry point;
+// it is fetched through the runtime so the library has no link-time dependency on libcuda.
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+static EncodeTiledFn encode_tiled_fn() {
+  static const EncodeTiledFn fn = [] {
+    void* f = nullptr;
+    cudaDriverEntryPointQueryResult q = cudaDriverEntryPointSymbolNotFound;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &f, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess) { cudaGetLastError(); f = nullptr; }
+    return reinterpret_cast<EncodeTiledFn>(f);
+  }();
+  return fn;
+}
+
+// One box = 64 token rows x 64 bf16 (128 bytes), 128-byte swizzle: exactly the canonical shared-memory
+// layout tcgen05.mma reads (K-major for K_t, MN-major for V_t^T).  Coordinates are (d, c1, c2):
+//   HND cache[page][head][token][d]:  dims (128, 64 tokens, page*Hkv + head)
+//   NHD cache[page][token][head][d]:  dims (128, Hkv, page*64 + token)
+// The outermost extent is not known to the ABI (the cache is the caller's); it is set to 2^30.
+static bool make_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  cuuint64_t dims[3]; cuuint64_t strides[2]; cuuint32_t box[3]; cuuint32_t es[3] = {1, 1, 1};
+  if (layout == ART_LAYOUT_HND) {
+    dims[0] = 128; dims[1] = 64; dims[2] = 1ull << 30;
+    strides[0] = 256; strides[1] = 256ull * 64;
+    box[0] = 64; box[1] = 64; box[2] = 1;
+  } else {
+    dims[0] = 128; dims[1] = static_cast<cuuint64_t>(Hkv); dims[2] = 1ull << 30;
+    strides[0] = 256; strides[1] = 256ull * Hkv;
+    box[0] = 64; box[1] = 1; box[2] = 64;
+  }
+  return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(base), dims, strides, box, es,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 static int validate(const art_desc_t* d, const void* q, const void* k, const void* v, const int32_t* bt,
@@ -856,14 +156,28 @@ static int mode_of(const art_desc_t* d, const art_thresholds_t* th) {
 }
 
 // shared-memory plan for a cluster size: as many ring stages as fit
-static LaunchPlan plan_for(int G, int PW, bool art, int C) {
+static LaunchPlan plan_for(bool tensor_core, int G, int PW, bool art, int C) {
   LaunchPlan pl;
   pl.C = C;
   pl.mslots = art ? (4 * C < 8 ? 8 : (4 * C > 32 ? 32 : 4 * C)) : 0;
   pl.stages = 6;
-  while (pl.stages > 2 && make_smem_map(G, PW, pl.stages, pl.mslots, art).total > static_cast<uint32_t>(kMaxSmem)) --pl.stages;
-  pl.smem = make_smem_map(G, PW, pl.stages, pl.mslots, art).total;
+  auto total = [&](int stages) {
+    return tensor_core ? tc::make_smem_map(G, PW, stages, pl.mslots, art).total
+                       : simt::make_smem_map(G, PW, stages, pl.mslots, art).total;
+  };
+  while (pl.stages > 2 && total(pl.stages) > static_cast<uint32_t>(kMaxSmem)) --pl.stages;
+  pl.smem = total(pl.stages);
   return pl;
+}
+
+static int fit_clusters(const art_desc_t* d, int G, int mode, int C, uint32_t smem) {
+  if (d->dtype == ART_DTYPE_BF16)
+    return dispatch(G, mode, [&](auto m, auto gg) {
+      return max_active_clusters(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value>, tc::kThreads, C, smem);
+    });
+  return dispatch(G, mode, [&](auto m, auto gg) {
+    return max_active_clusters(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>, simt::kThreads, C, smem);
+  });
 }
 
 // Cluster size: the largest C (<= 16) whose clusters for ALL groups can be co-resident, so every
@@ -873,17 +187,18 @@ static int choose_split(const art_desc_t* d, int mode, int* C_out) {
   const int groups = d->batch * d->num_kv_heads;
   const bool art = mode != 0;
   const int PW = mode == 2 ? d->head_dim : 32;
+  const bool tensor_core = d->dtype == ART_DTYPE_BF16;
   if (d->split != 0) { *C_out = d->split; return ART_OK; }
   int maxT = d->policy == ART_POLICY_LIST ? d->max_eligible : d->max_blocks_per_seq;
-  if (d->policy == ART_POLICY_SINK_WINDOW)
-    maxT = (d->sink_tokens + 63) / 64 + (d->window_tokens + 63) / 64 + 1 < maxT ? (d->sink_tokens + 63) / 64 + (d->window_tokens + 63) / 64 + 1 : maxT;
+  if (d->policy == ART_POLICY_SINK_WINDOW) {
+    const int sw = (d->sink_tokens + 63) / 64 + (d->window_tokens + 63) / 64 + 1;
+    maxT = sw < maxT ? sw : maxT;
+  }
   int best = 1;
   for (int C = 16; C >= 2; C >>= 1) {
     if (C > maxT) continue;
-    const LaunchPlan pl = plan_for(G, PW, art, C);
-    const int fit = dispatch(d->dtype, d->head_dim, G, mode, [&](auto m, auto t, auto dd, auto gg) {
-      return max_active_clusters<decltype(t), decltype(dd)::value, decltype(gg)::value, decltype(m)::value>(C, pl.smem);
-    });
+    const LaunchPlan pl = plan_for(tensor_core, G, PW, art, C);
+    const int fit = fit_clusters(d, G, mode, C, pl.smem);
     if (fit >= groups && fit > 0) { best = C; break; }
   }
   *C_out = best;
@@ -898,10 +213,11 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const int G = d->num_q_heads / d->num_kv_heads;
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
+  const bool tensor_core = d->dtype == ART_DTYPE_BF16;
   int C = 1;
   int rc = choose_split(d, mode, &C);
   if (rc != ART_OK) return rc;
-  const LaunchPlan pl = plan_for(G, PW, mode != 0, C);
+  const LaunchPlan pl = plan_for(tensor_core, G, PW, mode != 0, C);
 
   Params p = {};
   p.q = q; p.k = static_cast<const uint8_t*>(k); p.v = static_cast<const uint8_t*>(v);
@@ -921,9 +237,21 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   if (th) { p.tau = th->tau; p.phi = th->phi; p.patience = th->patience; }
   p.stages = pl.stages; p.mbox_slots = pl.mslots;
 
-  const cudaError_t e = static_cast<cudaError_t>(dispatch(d->dtype, d->head_dim, G, mode, [&](auto m, auto t, auto dd, auto gg) {
-    return static_cast<int>(launch_one<decltype(t), decltype(dd)::value, decltype(gg)::value, decltype(m)::value>(p, groups, C, pl.smem, stream));
-  }));
+  cudaError_t e;
+  if (tensor_core) {
+    CUtensorMap tmK, tmV;
+    if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
+      return ART_ERR_CUDA;
+    e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
+      return static_cast<int>(launch_cluster(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value>,
+                                             tc::kThreads, groups, C, pl.smem, stream, p, tmK, tmV));
+    }));
+  } else {
+    e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
+      return static_cast<int>(launch_cluster(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>,
+                                             simt::kThreads, groups, C, pl.smem, stream, p));
+    }));
+  }
   if (e != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
   return ART_OK;
 }
