@@ -270,6 +270,8 @@ def main():
     ap.add_argument("--impl", default="art", choices=["art", "reference"])
     ap.add_argument("--report", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
+                    help="time ONLY this arm of configs[1] (short command for ncu captures; prints a small JSON line)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "art" else args.warmup
 
@@ -302,6 +304,14 @@ def main():
     torch.cuda.synchronize()
     toks = eligible_tokens(w)
     peak, which = peaks()
+
+    if args.arm:
+        wa = wR if args.arm.startswith("R_") else w
+        kw = {"patience": art.ART_PATIENCE_INF} if args.arm == "pinf" else {}
+        r = measure(art, wa, args.steps, args.warmup, barrier, art_on=args.arm not in ("off", "R_off"), **kw)
+        r["arm"] = args.arm
+        print(json.dumps(r), flush=True)
+        return
 
     # ---- the timed region of the contract: exactly K ART-on steps on the literal config
     fn, out, stop, loaded = make_runner(art, w, art_on=True)
