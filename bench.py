@@ -270,6 +270,7 @@ def main():
     ap.add_argument("--impl", default="art", choices=["art", "reference"])
     ap.add_argument("--report", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--split", type=int, default=0, help="cluster size for --arm (0 = library default)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
                     help="time ONLY this arm of configs[1] (short command for ncu captures; prints a small JSON line)")
     args = ap.parse_args()
@@ -308,8 +309,10 @@ def main():
     if args.arm:
         wa = wR if args.arm.startswith("R_") else w
         kw = {"patience": art.ART_PATIENCE_INF} if args.arm == "pinf" else {}
-        r = measure(art, wa, args.steps, args.warmup, barrier, art_on=args.arm not in ("off", "R_off"), **kw)
+        r = measure(art, wa, args.steps, args.warmup, barrier, art_on=args.arm not in ("off", "R_off"),
+                    split=args.split, **kw)
         r["arm"] = args.arm
+        r["split"] = args.split or art.art_query_split(art.make_desc(wa), args.arm not in ("off", "R_off"))
         print(json.dumps(r), flush=True)
         return
 

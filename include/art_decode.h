@@ -74,8 +74,8 @@ typedef struct art_desc {
   int32_t max_eligible;        /* row stride of eligible_blocks (LIST) */
   float sm_scale;              /* logit scale; 0 => 1/sqrt(d) (Eq. 1) */
   int32_t split;               /* CTAs (thread-block cluster size) cooperating on one group:
-                                  0 = choose automatically, else 1, 2, 4, 8 or 16.  Any value gives the
-                                  same stop_block as the sequential algorithm. */
+                                  0 = choose automatically, else 1..16 (a power of two for F32).  Any value
+                                  gives the same stop_block as the sequential algorithm. */
   const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
   int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
                                   (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */

@@ -17,6 +17,7 @@ constexpr int kRowBytes = 256;                    // one token row of one head: 
 constexpr int kTileBytes = kBlockTokens * kRowBytes;   // 16 KiB: K or V tile of one block
 constexpr int kStageBytes = 2 * kTileBytes;       // K + V
 constexpr int kMaxSmem = 232448;                  // 227 KiB usable per CTA on sm_100
+constexpr int kSmemTwoPerSm = 115712;              // (228 KiB - 2 x 1 KiB reserved) / 2: two CTAs share an SM
 constexpr float kNegInf = -INFINITY;
 
 struct Params {
@@ -77,6 +78,15 @@ __device__ __forceinline__ bool mbar_try_wait(uint32_t bar, uint32_t parity) {
                : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
   return ok != 0;
 }
+// non-blocking probe of a phase (try_wait may suspend the thread for a while before answering "no")
+__device__ __forceinline__ bool mbar_test_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile("{\n\t.reg .pred p;\n\t"
+               "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+               "selp.u32 %0, 1, 0, p;\n\t}"
+               : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+  return ok != 0;
+}
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint32_t bar, uint32_t parity) {
   uint32_t ok;
   asm volatile("{\n\t.reg .pred p;\n\t"
@@ -124,6 +134,9 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
 __device__ __forceinline__ uint2 lds64(uint32_t addr) {
   uint2 r; asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(r.x), "=r"(r.y) : "r"(addr));
   return r;
+}
+__device__ __forceinline__ float lds_f32(uint32_t addr) {
+  float v; asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr)); return v;
 }
 __device__ __forceinline__ float fast_exp2(float x) {       // ex2.approx: exp2(-inf) = +0
   float y; asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x)); return y;

@@ -5,6 +5,10 @@
 //   art_decode_tc.cuh    bf16 KV, head_dim 128: TMA tensor loads, tcgen05.mma with TMEM accumulators
 //   art_decode_simt.cuh  fp32 KV, head_dim 64:  TMA bulk loads, CUDA-core FMAs (1e-5 tolerance rules out TF32)
 // The ART-off entry point is the same kernel template with the detector compiled out.
+#include <array>
+#include <map>
+#include <mutex>
+#include <utility>
 #include "art_decode_simt.cuh"
 #include "art_decode_tc.cuh"
 
@@ -22,6 +26,9 @@ static void set_cluster_attr(cudaLaunchAttribute* attr, int C) {
 template <typename Kern>
 static cudaError_t prepare_kernel(Kern kern, int C, uint32_t smem_bytes) {
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes));
+  if (e != cudaSuccess) return e;
+  // two CTAs per SM need the whole unified L1/shared array configured as shared memory
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, static_cast<int>(cudaSharedmemCarveoutMaxShared));
   if (e != cudaSuccess) return e;
   if (C > 8) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
   return e;
@@ -129,7 +136,8 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
     if (d->max_eligible < 0) return ART_ERR_SHAPE;
   }
   if (d->policy == ART_POLICY_SINK_WINDOW && (d->sink_tokens < 0 || d->window_tokens < 0)) return ART_ERR_SHAPE;
-  if (d->split != 0 && d->split != 1 && d->split != 2 && d->split != 4 && d->split != 8 && d->split != 16) return ART_ERR_SHAPE;
+  if (d->split < 0 || d->split > 16) return ART_ERR_SHAPE;
+  if (d->dtype == ART_DTYPE_F32 && (d->split & (d->split - 1))) return ART_ERR_SHAPE;
   if (!(d->sm_scale >= 0.f) || isinf(d->sm_scale)) return ART_ERR_SHAPE;
   if (th) {
     if (th->patience < 1) return ART_ERR_SHAPE;
@@ -155,33 +163,69 @@ static int mode_of(const art_desc_t* d, const art_thresholds_t* th) {
   return (th->probe_dim == 0 || th->probe_dim == d->head_dim) ? 2 : 1;
 }
 
-// shared-memory plan for a cluster size: as many ring stages as fit
+// shared-memory plan for a cluster size
 static LaunchPlan plan_for(bool tensor_core, int G, int PW, bool art, int C) {
   LaunchPlan pl;
   pl.C = C;
+  if (tensor_core) {
+    // Two CTAs per SM (3-stage ring each) unless the probe is the full output (MODE 2: bigger mailbox rows,
+    // more registers in the scan warp), which runs one CTA per SM with a deeper ring.
+    const bool two_per_sm = !art || PW == 32;
+    const uint32_t budget = two_per_sm ? kSmemTwoPerSm : static_cast<uint32_t>(kMaxSmem);
+    pl.stages = two_per_sm ? 3 : tc::kMaxStages;
+    pl.mslots = art ? 16 : 0;
+    auto total = [&]() { return tc::make_smem_map(G, PW, pl.stages, pl.mslots, art).total; };
+    if (art && total() > budget) pl.mslots = kScanBatch;           // the mailbox must hold one scan batch
+    while (pl.stages > 2 && total() > budget) --pl.stages;
+    pl.smem = total();
+    return pl;
+  }
   pl.mslots = art ? (4 * C < 8 ? 8 : (4 * C > 32 ? 32 : 4 * C)) : 0;
   pl.stages = 6;
-  auto total = [&](int stages) {
-    return tensor_core ? tc::make_smem_map(G, PW, stages, pl.mslots, art).total
-                       : simt::make_smem_map(G, PW, stages, pl.mslots, art).total;
-  };
+  auto total = [&](int stages) { return simt::make_smem_map(G, PW, stages, pl.mslots, art).total; };
   while (pl.stages > 2 && total(pl.stages) > static_cast<uint32_t>(kMaxSmem)) --pl.stages;
   pl.smem = total(pl.stages);
   return pl;
 }
 
-static int fit_clusters(const art_desc_t* d, int G, int mode, int C, uint32_t smem) {
-  if (d->dtype == ART_DTYPE_BF16)
-    return dispatch(G, mode, [&](auto m, auto gg) {
+// The occupancy calculator counts a kernel that allocates tensor memory as one CTA per SM, whatever it
+// allocates; the hardware runs two of ours side by side (256 of the SM's 512 columns each; checked with a
+// timestamp probe).  This twin has the same launch shape and no tcgen05 code: it is only ever passed to the
+// occupancy calculator, never launched.
+__global__ void __launch_bounds__(tc::kThreads, 2) tc_occupancy_twin(int* sink) {
+  extern __shared__ uint8_t twin_smem[];
+  if (sink) *sink = twin_smem[0];
+}
+
+// clusters of size C that can be co-resident, cached per (device, kernel class, shared memory size)
+static int cluster_capacity(const art_desc_t* d, int G, int mode, int C, uint32_t smem) {
+  static std::mutex mu;
+  static std::map<std::array<int, 4>, int> cache;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 0; }
+  const bool tensor_core = d->dtype == ART_DTYPE_BF16;
+  const bool twin = tensor_core && mode != 2;
+  const std::array<int, 4> key = {dev, twin ? -1 : (tensor_core ? 100 : 0) + G * 4 + mode, C, static_cast<int>(smem)};
+  std::lock_guard<std::mutex> lock(mu);
+  auto it = cache.find(key);
+  if (it != cache.end()) return it->second;
+  int fit;
+  if (twin) fit = max_active_clusters(tc_occupancy_twin, tc::kThreads, C, smem);
+  else if (tensor_core)
+    fit = dispatch(G, mode, [&](auto m, auto gg) {
       return max_active_clusters(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value>, tc::kThreads, C, smem);
     });
-  return dispatch(G, mode, [&](auto m, auto gg) {
-    return max_active_clusters(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>, simt::kThreads, C, smem);
-  });
+  else
+    fit = dispatch(G, mode, [&](auto m, auto gg) {
+      return max_active_clusters(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>, simt::kThreads, C, smem);
+    });
+  cache[key] = fit;
+  return fit;
 }
 
 // Cluster size: the largest C (<= 16) whose clusters for ALL groups can be co-resident, so every
-// group streams from the first cycle; never more CTAs than a group could have blocks.
+// group streams from the first cycle; never more CTAs than a group could have blocks.  The tensor-core
+// kernel takes any C (steps are dealt round-robin); the CUDA-core kernel's mailbox wants a power of two.
 static int choose_split(const art_desc_t* d, int mode, int* C_out) {
   const int G = d->num_q_heads / d->num_kv_heads;
   const int groups = d->batch * d->num_kv_heads;
@@ -195,10 +239,11 @@ static int choose_split(const art_desc_t* d, int mode, int* C_out) {
     maxT = sw < maxT ? sw : maxT;
   }
   int best = 1;
-  for (int C = 16; C >= 2; C >>= 1) {
+  for (int C = 16; C >= 2; --C) {
     if (C > maxT) continue;
+    if (!tensor_core && (C & (C - 1))) continue;
     const LaunchPlan pl = plan_for(tensor_core, G, PW, art, C);
-    const int fit = fit_clusters(d, G, mode, C, pl.smem);
+    const int fit = cluster_capacity(d, G, mode, C, pl.smem);
     if (fit >= groups && fit > 0) { best = C; break; }
   }
   *C_out = best;

@@ -1,73 +1,87 @@
 // ART decode attention, Blackwell tensor-core kernel (bf16 KV, head_dim 128): tcgen05 + TMEM + TMA.
 //
 // One thread-block CLUSTER of C CTAs per query group (sequence b, KV head g); traversal steps
-// t = 1..T are dealt round-robin, CTA c owns steps c+1, c+1+C, ...  Inside a CTA
-// one 64-token KV block is one pipeline item, handled by specialised warps that only meet through
-// mbarriers:
+// t = 1..T are dealt round-robin, CTA c owns steps c+1, c+1+C, ...  Two CTAs fit on
+// one SM (3-stage ring, 256 TMEM columns each), so one SM always has ~6 KV blocks in flight.  Inside a
+// CTA one 64-token KV block is one pipeline item, handled by specialised warps that meet only through
+// mbarriers, each warp waiting on ONE barrier at a time:
 //
-//   producer  (warp 0)     A1/A2  resolves block -> page, issues 4 TMA tensor boxes (K, V: two
-//                                 64-column halves each, 128-byte swizzle) into a ring of stages
-//   MMA       (warp 1, 1 thread)  A3  S[token, head]  = K_t . Q^T      tcgen05.mma M128 N16 K16 x8
-//                                 A5  PV[d, head]     = V_t^T . P^T    tcgen05.mma M128 N16 K16 x8
-//                                 both with fp32 accumulators in TENSOR MEMORY
-//   softmax   (warps 4-7)  A4     two groups of two warps (even / odd blocks), one thread per token:
-//                                 tcgen05.ld S, running max, p = 2^(s-m); p is split into bf16 hi + lo
-//                                 (keeps ~16 mantissa bits, so the probe of P~V_t is accurate to ~1e-5
-//                                 and the criterion does not flip) and written to shared memory as the
-//                                 B operand of the P.V MMA.  Each group is its own online-softmax stream.
-//   fold      (warps 8-11) A5/A6  one thread per output coordinate: tcgen05.ld P~V_t, publishes the
-//                                 step summary (reference max, block sum, probe components of P~V_t)
-//                                 to the cluster leader's mailbox (st.async + mbarrier complete_tx, no
-//                                 fences), and folds P~V_t into the running accumulator only once the
-//                                 leader has decided that step t <= t*
-//   scan      (warp 2, leader CTA)  A6/A7/A9  replays Algorithm 1 (Eq. 2-3)
-//                                 sequentially over the step summaries, broadcasts progress / t*
+//   producer (warp 0)      A1/A2  resolves block -> page, issues 4 TMA tensor boxes (K, V: two 64-column
+//                                 halves each, 128-byte swizzle) into the ring of stages
+//   S-MMA    (warp 1, 1 thr) A3   S[token, head] = K_t . Q^T : tcgen05.mma M128 N16 K16, issued twice per
+//                                 k-step so that tokens 0-31 and 32-63 of the block land in the SAME 32
+//                                 TMEM lanes (columns +0 / +16) of the softmax warp that owns the block
+//   softmax  (warps 4-7)   A4     warp q owns blocks i = q (mod 4): one warp sees all 64 tokens (two per
+//                                 thread), so the block maximum is one redux per head and no warp ever
+//                                 waits for another.  p = 2^(s - m_blk) relative to the BLOCK maximum (the
+//                                 warps are stateless), split into bf16 hi + lo (~16 mantissa bits, so the
+//                                 probe of P~V_t is accurate to ~1e-5 and the criterion does not flip) and
+//                                 written to shared memory as the B operand of the P.V MMA
+//   PV-MMA   (warp 3, 1 thr) A5   PV[d, head] = V_t^T . P^T : tcgen05.mma M128 N16 K16 x 4 x (hi, lo)
+//   fold     (warps 8-11)  A5/A6  one thread per output coordinate: tcgen05.ld of P~V_t; publishes the step
+//                                 summary (m_blk, block sum, probe components of P~V_t) to the cluster
+//                                 leader's mailbox (st.async + mbarrier complete_tx, no fences) and merges
+//                                 P~V_t into the running (m, l, acc) only once the leader has decided that
+//                                 step t <= t*
+//   scan     (warp 2, leader CTA)  A6/A7/A9  replays Algorithm 1 (Eq. 2-3) sequentially
+//                                 over the step summaries (art_scan.cuh), broadcasts progress / t*
 //
-// The block-local P~V_t of up to 16 steps wait UNFOLDED in tensor memory (16 x 16 columns), so the
-// loads, the MMAs and the softmax never wait for the sequential decision; blocks with step > t* are
-// simply never folded, which makes the result equal to the sequential algorithm's for any C.
+// The block-local P~V_t of up to 8 steps per CTA wait UNFOLDED in tensor memory, so loads, MMAs and
+// softmax never wait for the sequential decision; blocks with step > t* are simply never folded, which
+// makes the result equal to the sequential algorithm's for any C.
 #pragma once
 #include <cuda.h>   // CUtensorMap (type only: the encoder is fetched through the runtime, no -lcuda)
 
 #include "art_common.cuh"
+#include "art_scan.cuh"
 
 namespace art {
 namespace tc {
 
 constexpr int kThreads = 384;
-constexpr int kWarpProducer = 0, kWarpMma = 1, kWarpScan = 2, kWarpTmem = 3, kWarpSoftmax0 = 4, kWarpFold0 = 8;
+// Fold and softmax warps must sit at warp % 4 == TMEM lane quadrant.  The single-thread roles and the scan warp
+// get the highest warp ids: the SM's schedulers favour them, and their latency is what the pipeline feels.
+constexpr int kWarpFold0 = 0, kWarpSoftmax0 = 4, kWarpProducer = 8, kWarpMmaS = 9, kWarpMmaPV = 10, kWarpScan = 11;
 constexpr int kD = 128;                      // head_dim
 constexpr int kUmmaN = 16;                   // MMA N: the group's heads padded to 16
-constexpr int kSSlots = 4;                   // S accumulators in flight (16 TMEM columns each)
-constexpr int kPVSlots = 16;                 // unfolded P~V_t results (16 TMEM columns each)
-constexpr int kTmemCols = 512;
+constexpr int kSSlots = 4;                   // S accumulators: one per softmax warp, 2 x 16 TMEM columns
+constexpr int kSCols = 2 * kUmmaN;
+constexpr int kPVSlots = 8;                  // unfolded P~V_t results (16 TMEM columns each)
+constexpr int kTmemCols = 256;               // 4 x 32 + 8 x 16; two CTAs share the SM's 512 columns
+constexpr int kIterSlots = 16;               // softmax -> fold hand-over ring; >= kPVSlots + max stages
+constexpr int kMaxStages = 6;
 constexpr int kBoxBytes = 8192;              // one TMA box: 64 rows x 128 bytes
-constexpr int kQLbo = 256, kQSbo = 128;      // Q^T as B operand: [16 d-chunks][16 rows][16 B]
-constexpr int kQBytes = 16 * kQLbo;
-constexpr int kPLbo = 272, kPSbo = 128;      // P^T as B operand: [8 token-chunks][16 rows][16 B] (+16 B pad:
-constexpr int kPBufBytes = 2304;             //   the 4 chunks a warp writes fall into distinct banks)
+constexpr int kFront = 12288;                // mapped bytes the S MMA may read below a K tile (3 x 32 rows)
+// Q^T as B operand (K-major, no swizzle): [16 d-chunks of 8][rows][16 B], chunk stride 128 B.  Rows 8-15 of
+// a chunk alias rows 0-7 of the next one: they only feed accumulator columns >= 8, which nobody reads.
+constexpr int kQLbo = 128, kQSbo = 128, kQBytes = 16 * kQLbo + 128;
+static_assert(kIterSlots >= kPVSlots + kMaxStages, "IterSlot ring too short");
 
-struct IterSlot {            // what softmax hands to fold for one block (ring of kPVSlots)
-  float alpha[8];            // 2^(m_old - m_new): rescale of everything its stream folded before this block
-  float mref[8];             // m_new: reference exponent of this block's p (log2 domain)
-  float lsum[2][8];          // per softmax warp: sum of the block's (rounded) p
+// P^T as B operand: [8 token-chunks of 8][rows][16 B]; chunk stride 16 G + 16 B puts the 4 chunks a warp
+// writes at once into distinct banks; rows >= G alias later chunks (unread accumulator columns).
+__host__ __device__ constexpr int p_lbo(int G) { return 16 * G + 16; }
+__host__ __device__ constexpr int p_buf_bytes(int G) { return 7 * p_lbo(G) + 256; }
+
+struct IterSlot {            // what softmax hands to fold for one block
+  float mref[8];             // m_blk: block maximum of the scaled logits (log2 domain) = reference of p
+  float lsum[8];             // sum of the block's (rounded) p
 };
 
 struct SmemMap {
-  uint32_t qb, pb, slots, sinfo, xchg, mbox, bars, misc, ring, total;
-  uint32_t full0, empty0, sfull0, sfree0, pfull0, pvfull0, pvfree0, xchg0, done0, mbox0, nbars;
+  uint32_t qb, pb, slots, sinfo, mbox, bars, misc, ring, total;
+  uint32_t full0, empty0, pfull0, sfull0, sfree0, pvfull0, pvfree0, done0, mbox0, nbars;
 };
 
-// Offsets from a 1024-byte aligned base.  The small buffers come first: the S MMA of odd blocks reads
-// 8 KiB below its K tile (rows that only feed unused accumulator lanes), which must be mapped memory.
+// Offsets from the (1024-byte aligned) dynamic shared memory base.  The small buffers come first: the S MMA
+// reads up to kFront bytes below its K tile (rows that only feed unused accumulator lanes).
 __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int mslots, bool art) {
   SmemMap m;
   uint32_t off = 0;
   m.qb = off; off += kQBytes;
-  m.pb = off; off += static_cast<uint32_t>(stages) * 2u * kPBufBytes;
-  m.slots = off; off += kPVSlots * static_cast<uint32_t>(sizeof(IterSlot));
-  m.sinfo = off; off += static_cast<uint32_t>(stages) * 16u;
-  m.xchg = off; off += 2u * 2u * 2u * 8u * 4u;
+  m.pb = off; off += static_cast<uint32_t>(stages) * 2u * p_buf_bytes(G);
+  m.slots = off; off += kIterSlots * static_cast<uint32_t>(sizeof(IterSlot));
+  m.sinfo = off; off += static_cast<uint32_t>(stages) * 8u;
+  off = (off + 15u) & ~15u;                // mailbox rows are written with 16-byte st.async
   m.mbox = off; off += art ? static_cast<uint32_t>(mslots) * G * (2 + PW) * 4u : 0u;
   off = (off + 15u) & ~15u;
   m.bars = off;
@@ -75,15 +89,15 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   m.full0 = n; n += stages; m.empty0 = n; n += stages; m.pfull0 = n; n += stages;
   m.sfull0 = n; n += kSSlots; m.sfree0 = n; n += kSSlots;
   m.pvfull0 = n; n += kPVSlots; m.pvfree0 = n; n += kPVSlots;
-  m.xchg0 = n; n += 4; m.done0 = n; n += 1;
+  m.done0 = n; n += 2;
   m.mbox0 = n; n += art ? mslots : 0;
   m.nbars = n;
   off += n * 8u;
   m.misc = off; off += 128u;             // ctrl, loaded, tmem_ptr, cta_m[8], cta_l[8]
   off = (off + 1023u) & ~1023u;
-  if (off < 8192u) off = 8192u;
+  if (off < static_cast<uint32_t>(kFront)) off = kFront;
   m.ring = off; off += static_cast<uint32_t>(stages) * kStageBytes;
-  m.total = off + 1024u;                 // + slack: the base is aligned to 1024 B at run time
+  m.total = off;
   return m;
 }
 constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8, kCtaM = 32, kCtaL = 64;
@@ -170,29 +184,57 @@ __device__ __forceinline__ int ld_ctrl_relaxed(uint32_t addr) {
   int v; asm volatile("ld.relaxed.cluster.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
 }
 
+// Sum G per-lane values over the 32 lanes with a transposing butterfly (G-1 + 5-log2(G) ... shuffles instead
+// of 5 G): afterwards v[0] of lane l holds the total of value head_of_lane32<G>(l).
+template <int N, int MASK>
+struct Reduce32 {
+  static __device__ __forceinline__ void run(float* v, int lane) {
+    if constexpr (N > 1) {
+      constexpr int n = N / 2;
+      const bool up = (lane & MASK) != 0;
+#pragma unroll
+      for (int i = 0; i < n; ++i) {
+        const float keep = up ? v[i + n] : v[i];
+        const float send = up ? v[i] : v[i + n];
+        v[i] = keep + __shfl_xor_sync(0xffffffffu, send, MASK);
+      }
+      if constexpr (MASK > 1) Reduce32<n, MASK / 2>::run(v, lane);
+    } else {
+      v[0] += __shfl_xor_sync(0xffffffffu, v[0], MASK);
+      if constexpr (MASK > 1) Reduce32<1, MASK / 2>::run(v, lane);
+    }
+  }
+};
+template <int G> __device__ __forceinline__ int head_of_lane32(int lane) {
+  int h = 0;
+  if constexpr (G >= 2) h += ((lane >> 4) & 1) * (G / 2);
+  if constexpr (G >= 4) h += ((lane >> 3) & 1) * (G / 4);
+  if constexpr (G >= 8) h += ((lane >> 2) & 1) * (G / 8);
+  return h;
+}
+
 // ----------------------------------------------------------------------------- the kernel
 
 // MODE 0: ART off.  MODE 1: ART on, probe = 32 coordinates k*(d/32).  MODE 2: ART on, probe = all d.
 template <int G, int MODE>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __launch_bounds__(kThreads, (MODE == 2) ? 1 : 2)
 art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
   constexpr bool ART = MODE != 0;
   constexpr int PW = (MODE == 2) ? kD : 32;          // probe width m
   constexpr int NP = kPVSlots, NS = kSSlots;
+  constexpr int LBO_P = p_lbo(G), PBUF = p_buf_bytes(G);
   constexpr uint32_t kSummaryBytes = (2 + PW) * G * 4;   // mailbox row block of one step: [2 + PW][G] floats
-  static_assert((NP & (NP - 1)) == 0 && (NS & (NS - 1)) == 0, "slot rings are indexed with masks");
 
-  extern __shared__ uint8_t smem_raw[];
+  extern __shared__ __align__(1024) uint8_t smem[];
   const int S = p.stages, M = p.mbox_slots;
   const SmemMap sm = make_smem_map(G, PW, S, M, ART);
-  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  uint8_t* smem = smem_raw + (sbase - smem_u32(smem_raw));
+  const uint32_t sbase = smem_u32(smem);
+  if ((sbase & 1023u) != 0u) __trap();               // the 128-byte swizzle pattern is address based
   const uint32_t bars = sbase + sm.bars;
   auto bar = [&](uint32_t idx) { return bars + idx * 8u; };
   const uint32_t a_ctrl = sbase + sm.misc + kCtrl, a_loaded = sbase + sm.misc + kLoaded, a_tmem = sbase + sm.misc + kTmemPtr;
   IterSlot* slots = reinterpret_cast<IterSlot*>(smem + sm.slots);
-  unsigned long long* sinfo = reinterpret_cast<unsigned long long*>(smem + sm.sinfo);   // [S][2]: mask, pad
-  float* xchg = reinterpret_cast<float*>(smem + sm.xchg);                               // [group][parity][warp][8]
+  unsigned long long* sinfo = reinterpret_cast<unsigned long long*>(smem + sm.sinfo);   // [S] token masks
   float* mbox = reinterpret_cast<float*>(smem + sm.mbox);
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -205,13 +247,12 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   const int Tn = tr.T;
   const int n_c = (Tn > rank) ? (Tn - rank + C - 1) / C : 0;   // steps owned by this CTA
 
-  // ---- one-time setup: barriers, tensor memory, Q^T and the zero padding rows of P^T
+  // ---- one-time setup: barriers, tensor memory, Q^T
   if (tid == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 64); }
-    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 2); }
+    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 32); }
+    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 1); }
     for (int s = 0; s < NP; ++s) { mbar_init(bar(sm.pvfull0 + s), 1); mbar_init(bar(sm.pvfree0 + s), 4); }
-    for (int s = 0; s < 4; ++s) mbar_init(bar(sm.xchg0 + s), 2);
-    mbar_init(bar(sm.done0), 1);
+    mbar_init(bar(sm.done0), 1); mbar_init(bar(sm.done0 + 1), 1);
     if (ART) {
       for (int s = 0; s < M; ++s) {
         mbar_init(bar(sm.mbox0 + s), 1);
@@ -221,23 +262,24 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_loaded, 0);
     fence_mbar_init();
   }
-  if (warp == kWarpTmem) tmem_alloc(a_tmem, kTmemCols);
+  if (warp == kWarpMmaPV) tmem_alloc(a_tmem, kTmemCols);
   {
     const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * G) * kD;
-    for (int idx = tid; idx < 16 * kD; idx += kThreads) {
+    for (int idx = tid; idx < 8 * kD; idx += kThreads) {       // rows >= G: zeros (rows 8-15 alias, see kQLbo)
       const int row = idx / kD, dc = idx % kD;
       const __nv_bfloat16 v = (row < G) ? qp[row * kD + dc] : __float2bfloat16_rn(0.f);
       *reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + (dc >> 3) * kQLbo + row * 16 + (dc & 7) * 2) = v;
     }
-    uint4* pz = reinterpret_cast<uint4*>(smem + sm.pb);
-    for (int idx = tid; idx < S * 2 * kPBufBytes / 16; idx += kThreads) pz[idx] = make_uint4(0u, 0u, 0u, 0u);
+    if (tid < 64) reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + 16 * kQLbo)[tid] = __float2bfloat16_rn(0.f);
+    uint4* pz = reinterpret_cast<uint4*>(smem + sm.pb);        // P^T rows are read before they are first written
+    for (int idx = tid; idx < S * 2 * PBUF / 16; idx += kThreads) pz[idx] = make_uint4(0u, 0u, 0u, 0u);
   }
-  fence_proxy_async();          // Q^T / P^T padding written by threads, read by the tensor core
+  fence_proxy_async();          // Q^T written by threads, read by the tensor core
   tc_fence_before();
   cluster_sync_all();           // barriers of every CTA of the cluster are live before any remote store
   tc_fence_after();
   const uint32_t tmem_base = static_cast<uint32_t>(ld_volatile_s32(a_tmem));
-  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kUmmaN;
+  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kSCols;
 
   // "fired and step t lies beyond t*": every wait that could otherwise never end checks this
   auto beyond_stop = [&](int t) -> bool {
@@ -251,13 +293,12 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   };
   auto step_of = [&](int i) { return i * C + rank + 1; };
 
-  // fold warps: this thread's output coordinate and the running (un-normalised) state of the two
-  // softmax streams (even / odd blocks); read by the epilogue
-  const int fq = (warp - kWarpFold0) & 3;
+  // fold warps: this thread's output coordinate and the running (un-normalised) state; read by the epilogue
+  const int fq = warp & 3;
   const int d = fq * 32 + lane;                               // output coordinate == TMEM lane
-  float acc0[G], acc1[G], m0[G], m1[G], l0[G], l1[G];
+  float acc[G], m_tot[G], l_tot[G];
 #pragma unroll
-  for (int h = 0; h < G; ++h) { acc0[h] = acc1[h] = 0.f; m0[h] = m1[h] = kNegInf; l0[h] = l1[h] = 0.f; }
+  for (int h = 0; h < G; ++h) { acc[h] = 0.f; m_tot[h] = kNegInf; l_tot[h] = 0.f; }
 
   if (warp == kWarpProducer) {
     // ===================================================== A1 + A2: resolve blocks, issue TMA loads
@@ -287,7 +328,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (lane == 0) {
           const uint32_t fb = bar(sm.full0 + stage);
           const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
-          sinfo[stage * 2] = mask_k;
+          sinfo[stage] = mask_k;
           if (mask_k == 0ull) {
             mbar_arrive(fb);                                 // nothing to load: an all-masked step
           } else {
@@ -306,147 +347,178 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     if (lane == 0) st_volatile_s32(a_loaded, loaded);
     // drain: tensor copies still in flight must land before the CTA reuses the ring or exits (H5)
     for (int j = max(0, it_issued - S); j < it_issued; ++j) mbar_wait(bar(sm.full0 + j % S), (j / S) & 1);
-  } else if (warp == kWarpMma) {
-    // ===================================================== A3 + A5: the two MMAs of every block
+  } else if (warp == kWarpMmaS) {
+    // ===================================================== A3: S = K_t Q^T, rows = tokens, columns = heads
     if (lane == 0) {
       const uint64_t dK = kDescSw128 | desc_strides(16, 1024);         // K tile, K-major, 128-B swizzle
-      const uint64_t dV = kDescSw128 | desc_strides(kBoxBytes, 1024);  // V tile as V^T: MN-major, 128-B swizzle
       const uint64_t dQ = kDescNoSw | desc_strides(kQLbo, kQSbo);
-      const uint64_t dP = kDescNoSw | desc_strides(kPLbo, kPSbo);
       const uint32_t qb = sbase + sm.qb;
-      int si = 0, pi = 0;                                     // next block whose S / P.V MMAs are to be issued
-      int s_st = 0, p_st = 0; uint32_t s_ph = 0, p_ph = 0;    // their ring stage and (i / S) & 1
-      while (pi < n_c) {
-        bool did = false;
-        if (si < n_c && mbar_try_wait(bar(sm.full0 + s_st), s_ph) &&
-            (si < NS || mbar_try_wait(bar(sm.sfree0 + (si & (NS - 1))), ((si / NS) - 1) & 1))) {
-          // S = K_t Q^T: rows = tokens, columns = heads.  M = 128 rows are read starting 8 KiB BELOW the K tile
-          // for odd blocks, so their 64 tokens land in TMEM lanes 64-127 (softmax group 1); the other 64 rows
-          // are whatever lies next to the tile and only feed lanes nobody reads.
-          tc_fence_after();
-          const uint32_t kt = sbase + sm.ring + s_st * kStageBytes - ((si & 1) ? kBoxBytes : 0);
+      int st = 0; uint32_t ph = 0;
+      for (int i = 0; i < n_c; ++i) {
+        const int q = i & (NS - 1), t = step_of(i);
+        if (!wait_or_stop(bar(sm.full0 + st), ph, t)) break;
+        if (i >= NS && !wait_or_stop(bar(sm.sfree0 + q), ((i / NS) - 1) & 1, t)) break;
+        tc_fence_after();
+        // M = 128 rows are read starting 32 q token rows BELOW the tile (tokens 0-31 -> TMEM lanes 32q..32q+31,
+        // columns +0) and once more 32 rows further up (tokens 32-63 -> the same lanes, columns +16).  The
+        // other 96 rows are whatever lies next to the tile and only feed lanes nobody reads.
+        const uint32_t kt = sbase + sm.ring + st * kStageBytes - q * 4096;
+        const uint32_t dcol = tmem_S + q * kSCols;
 #pragma unroll
-          for (int ks = 0; ks < 8; ++ks)                      // 8 x 16 = head_dim
-            umma_bf16(tmem_S + (si & (NS - 1)) * kUmmaN, dK | desc_addr(kt + (ks >> 2) * kBoxBytes + (ks & 3) * 32),
-                      dQ | desc_addr(qb + ks * 2 * kQLbo), kIdescS, ks > 0);
-          umma_commit(bar(sm.sfull0 + (si & (NS - 1))));
-          ++si; if (++s_st == S) { s_st = 0; s_ph ^= 1u; }
-          did = true;
+        for (int ks = 0; ks < 8; ++ks) {                      // 8 x 16 = head_dim
+          const uint32_t ka = kt + (ks >> 2) * kBoxBytes + (ks & 3) * 32;
+          const uint64_t bq = dQ | desc_addr(qb + ks * 2 * kQLbo);
+          umma_bf16(dcol, dK | desc_addr(ka), bq, kIdescS, ks > 0);
+          umma_bf16(dcol + kUmmaN, dK | desc_addr(ka + 4096), bq, kIdescS, ks > 0);
         }
-        if (pi < si && mbar_try_wait(bar(sm.pfull0 + p_st), p_ph) &&
-            (pi < NP || mbar_try_wait(bar(sm.pvfree0 + (pi & (NP - 1))), ((pi / NP) - 1) & 1))) {
-          // P~V_t = V_t^T P^T: rows = d, columns = heads; p = hi + lo
-          tc_fence_after();
-          const uint32_t vt = sbase + sm.ring + p_st * kStageBytes + 2 * kBoxBytes;
-          const uint32_t pb = sbase + sm.pb + p_st * 2 * kPBufBytes;
-#pragma unroll
-          for (int part = 0; part < 2; ++part)
-#pragma unroll
-            for (int ks = 0; ks < 4; ++ks)                    // 4 x 16 = tokens of the block
-              umma_bf16(tmem_PV + (pi & (NP - 1)) * kUmmaN, dV | desc_addr(vt + ks * 2048),
-                        dP | desc_addr(pb + part * kPBufBytes + ks * 2 * kPLbo), kIdescPV, (part | ks) > 0);
-          umma_commit(bar(sm.empty0 + p_st));                 // K/V stage and its P buffer are free again
-          umma_commit(bar(sm.pvfull0 + (pi & (NP - 1))));
-          ++pi; if (++p_st == S) { p_st = 0; p_ph ^= 1u; }
-          did = true;
-        }
-        if (!did && beyond_stop(step_of(pi))) break;          // every block <= t* has had both MMAs
+        umma_commit(bar(sm.sfull0 + q));
+        if (++st == S) { st = 0; ph ^= 1u; }
       }
       umma_commit(bar(sm.done0));                             // every MMA retired before TMEM is released
       mbar_wait(bar(sm.done0), 0);
     }
-  } else if (warp >= kWarpSoftmax0 && warp < kWarpSoftmax0 + 4) {
-    // ===================================================== A4: online softmax, one thread per token
-    const int grp = (warp - kWarpSoftmax0) >> 1;              // stream: even / odd blocks
-    const int wq = (warp - kWarpSoftmax0) & 1;                // which 32 tokens of the block
-    const int tok = wq * 32 + lane;
-    const uint32_t tlane = static_cast<uint32_t>((warp - kWarpSoftmax0) * 32) << 16;   // TMEM lane quadrant == warp % 4
-    float m_run[G];
+  } else if (warp == kWarpMmaPV) {
+    // ===================================================== A5: P~V_t = V_t^T P^T, rows = d, columns = heads
+    if (lane == 0) {
+      const uint64_t dV = kDescSw128 | desc_strides(kBoxBytes, 1024);  // V tile as V^T: MN-major, 128-B swizzle
+      const uint64_t dP = kDescNoSw | desc_strides(LBO_P, 128);
+      int st = 0; uint32_t ph = 0;
+      for (int i = 0; i < n_c; ++i) {
+        const int ps = i & (NP - 1), t = step_of(i);
+        if (!wait_or_stop(bar(sm.pfull0 + st), ph, t)) break;
+        if (i >= NP && !wait_or_stop(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1, t)) break;
+        tc_fence_after();
+        const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
+        const uint32_t pb = sbase + sm.pb + st * 2 * PBUF;
 #pragma unroll
-    for (int h = 0; h < G; ++h) m_run[h] = kNegInf;
-    int s = grp % S; uint32_t ph = (grp / S) & 1;             // ring stage and (i / S) & 1 of block i
-    for (int i = grp, k = 0; i < n_c; i += 2, ++k) {
+        for (int part = 0; part < 2; ++part)                  // p = hi + lo
+#pragma unroll
+          for (int ks = 0; ks < 4; ++ks)                      // 4 x 16 = tokens of the block
+            umma_bf16(tmem_PV + ps * kUmmaN, dV | desc_addr(vt + ks * 2048),
+                      dP | desc_addr(pb + part * PBUF + ks * 2 * LBO_P), kIdescPV, (part | ks) > 0);
+        umma_commit(bar(sm.empty0 + st));                     // K/V stage and its P buffer are free again
+        umma_commit(bar(sm.pvfull0 + ps));
+        if (++st == S) { st = 0; ph ^= 1u; }
+      }
+      umma_commit(bar(sm.done0 + 1));
+      mbar_wait(bar(sm.done0 + 1), 0);
+    }
+  } else if (warp >= kWarpSoftmax0 && warp < kWarpSoftmax0 + 4) {
+    // ===================================================== A4: block-local softmax, two tokens per thread
+    const int q = warp - kWarpSoftmax0;                       // TMEM lane quadrant == warp % 4; owns blocks i = q (mod 4)
+    const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
+    int st = q % S;                                           // ring stage of block i
+    for (int i = q; i < n_c; i += NS) {
       const int t = step_of(i);
-      if (!wait_or_stop(bar(sm.sfull0 + (i & (NS - 1))), (i / NS) & 1, t)) break;
+      if (!wait_or_stop(bar(sm.sfull0 + q), (i / NS) & 1, t)) break;
       tc_fence_after();
-      float sc[G];
-      tmem_ld<G>(tmem_S + tlane + (i & (NS - 1)) * kUmmaN, sc);
+      float s0[G], s1[G];
+      tmem_ld<G>(taddr, s0);
+      tmem_ld<G>(taddr + kUmmaN, s1);
       tmem_ld_wait();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.sfree0 + (i & (NS - 1))));
-      const unsigned long long vmask = sinfo[s * 2];          // written before the loads the S MMA waited for
-      if (i >= NP && !wait_or_stop(bar(sm.pvfree0 + (i & (NP - 1))), ((i / NP) - 1) & 1, t)) break;   // IterSlot reuse
-      const bool valid = (vmask >> tok) & 1ull;
-      float wmax[G];
+      if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+      const unsigned long long vmask = sinfo[st];             // written before the loads the S MMA waited for
+      const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
+      float mb[G];
 #pragma unroll
       for (int h = 0; h < G; ++h) {
-        sc[h] = valid ? sc[h] * p.scale_log2 : kNegInf;       // masked tokens: weight 0 (R8); their K may be NaN
-        wmax[h] = warp_max_f32(sc[h]);
+        s0[h] = v0 ? s0[h] * p.scale_log2 : kNegInf;          // masked tokens: weight 0 (R8); their K may be NaN
+        s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
+        mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
       }
-      float* xw = xchg + (((grp * 2 + (k & 1)) * 2) + wq) * 8;
-#pragma unroll
-      for (int h = 0; h < G; ++h) if (lane == h) xw[h] = wmax[h];
-      __syncwarp();
-      const uint32_t xb = bar(sm.xchg0 + grp * 2 + (k & 1));
-      if (lane == 0) mbar_arrive(xb);
-      if (!wait_or_stop(xb, (k >> 1) & 1, t)) break;
-      const float* xo = xchg + (((grp * 2 + (k & 1)) * 2) + (wq ^ 1)) * 8;
-      __nv_bfloat16* pbh = reinterpret_cast<__nv_bfloat16*>(smem + sm.pb + s * 2 * kPBufBytes + (tok >> 3) * kPLbo + (tok & 7) * 2);
-      __nv_bfloat16* pbl = reinterpret_cast<__nv_bfloat16*>(reinterpret_cast<uint8_t*>(pbh) + kPBufBytes);
-      IterSlot& slot = slots[i & (NP - 1)];
+      uint8_t* pb0 = smem + sm.pb + st * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;   // token `lane`, row 0, hi
       float ls[G];
 #pragma unroll
       for (int h = 0; h < G; ++h) {
-        const float m_new = fmaxf(m_run[h], fmaxf(wmax[h], xo[h]));
-        const float pj = (valid && m_new != kNegInf) ? fast_exp2(sc[h] - m_new) : 0.f;
-        const __nv_bfloat16 hi = __float2bfloat16_rn(pj);
-        const __nv_bfloat16 lo = __float2bfloat16_rn(pj - __bfloat162float(hi));
-        pbh[h * 8] = hi; pbl[h * 8] = lo;                     // row h, 16 bytes per row
-        ls[h] = __bfloat162float(hi) + __bfloat162float(lo);  // the weight the tensor core really uses
-        if (lane == 0 && wq == 0) { slot.mref[h] = m_new; slot.alpha[h] = (m_new == kNegInf) ? 1.f : fast_exp2(m_run[h] - m_new); }
-        m_run[h] = m_new;
+        const float p0 = (v0 && mb[h] != kNegInf) ? fast_exp2(s0[h] - mb[h]) : 0.f;
+        const float p1 = (v1 && mb[h] != kNegInf) ? fast_exp2(s1[h] - mb[h]) : 0.f;
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(p0), h1 = __float2bfloat16_rn(p1);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(p0 - __bfloat162float(h0)), l1 = __float2bfloat16_rn(p1 - __bfloat162float(h1));
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16) = h0;
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + 4 * LBO_P) = h1;              // token lane + 32: 4 chunks on
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF) = l0;
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF + 4 * LBO_P) = l1;
+        // the weight the tensor core really uses
+        ls[h] = (__bfloat162float(h0) + __bfloat162float(l0)) + (__bfloat162float(h1) + __bfloat162float(l1));
       }
-      if (vmask != ~0ull && !valid) {                         // masked V rows may hold NaN: 0 * NaN would poison P~V
-        uint4* vr = reinterpret_cast<uint4*>(smem + sm.ring + s * kStageBytes + 2 * kBoxBytes + tok * 128);
+      if (vmask != ~0ull) {                                   // masked V rows may hold NaN: 0 * NaN would poison P~V
+        uint4* vr = reinterpret_cast<uint4*>(smem + sm.ring + st * kStageBytes + 2 * kBoxBytes);
+        if (!v0) {
 #pragma unroll
-        for (int c = 0; c < 8; ++c) { vr[c] = make_uint4(0u, 0u, 0u, 0u); vr[c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
+          for (int c = 0; c < 8; ++c) { vr[lane * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[lane * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
+        }
+        if (!v1) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) { vr[(lane + 32) * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[(lane + 32) * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
+        }
       }
+      // block sum per head: lane l ends up with the total of head head_of_lane32(l)
+      Reduce32<G, 16>::run(ls, lane);
+      {
+        const int hh = head_of_lane32<G>(lane);
+        float mine = mb[0];
 #pragma unroll
-      for (int o = 16; o >= 1; o >>= 1)
-#pragma unroll
-        for (int h = 0; h < G; ++h) ls[h] += __shfl_xor_sync(0xffffffffu, ls[h], o);
-#pragma unroll
-      for (int h = 0; h < G; ++h) if (lane == h) slot.lsum[wq][h] = ls[h];
+        for (int h = 1; h < G; ++h) mine = (hh == h) ? mb[h] : mine;
+        IterSlot& slot = slots[i & (kIterSlots - 1)];
+        if ((lane & (32 / G - 1)) == 0) { slot.mref[hh] = mine; slot.lsum[hh] = ls[0]; }
+      }
       fence_proxy_async();                                    // P^T (and V fixes) visible to the tensor core
-      mbar_arrive(bar(sm.pfull0 + s));
-      s += 2; if (s >= S) { s -= S; ph ^= 1u; }
+      mbar_arrive(bar(sm.pfull0 + st));
+      st += NS; while (st >= S) st -= S;
     }
-    (void)ph;
-  } else if (warp >= kWarpFold0) {
-    // ===================================================== A5 / A6: publish step summaries, fold P~V_t
+  } else if (warp < kWarpFold0 + 4) {
+    // ===================================================== A5 / A6: publish step summaries, merge P~V_t
     const uint32_t tlane = static_cast<uint32_t>(fq * 32) << 16;
-    int pub = 0, fld = 0;
-    while (fld < n_c) {
-      const int c = ART ? ld_ctrl_relaxed(a_ctrl) : 0;
-      if (ART && c < 0 && step_of(fld) > -c) break;           // everything from here on lies beyond t*
-      if constexpr (ART) {
-        // ---- publish the summary of the next finished block (does not wait for any decision)
-        if (pub < n_c && pub - fld < NP && mbar_try_wait(bar(sm.pvfull0 + (pub & (NP - 1))), (pub / NP) & 1)) {
+    // merge block i (its P~V_t is relative to its own block maximum) into the running state
+    auto fold = [&](int i) {
+      tc_fence_after();
+      float pv[G];
+      tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN, pv);
+      tmem_ld_wait();
+      const IterSlot& sl = slots[i & (kIterSlots - 1)];
+#pragma unroll
+      for (int h = 0; h < G; ++h) {
+        const float mr = sl.mref[h];
+        if (mr != kNegInf) {                                  // a block with no valid token changes nothing
+          const float mn = fmaxf(m_tot[h], mr);
+          const float a = fast_exp2(m_tot[h] - mn), bb = fast_exp2(mr - mn);
+          acc[h] = fmaf(a, acc[h], bb * pv[h]);
+          l_tot[h] = fmaf(a, l_tot[h], bb * sl.lsum[h]);
+          m_tot[h] = mn;
+        }
+      }
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(sm.pvfree0 + (i & (NP - 1))));
+    };
+    if constexpr (!ART) {
+      for (int i = 0; i < n_c; ++i) {
+        mbar_wait(bar(sm.pvfull0 + (i & (NP - 1))), (i / NP) & 1);
+        fold(i);
+      }
+    } else {
+      int pub = 0, fld = 0;
+      bool pub_ready = false;                                 // P~V of block `pub` is complete in tensor memory
+      while (fld < n_c) {
+        const int c = ld_ctrl_relaxed(a_ctrl);
+        if (c < 0 && step_of(fld) > -c) break;                // everything from here on lies beyond t*
+        // ---- merge the oldest unfolded block once the decision for the steps before it is known
+        if (fld < pub && (c < 0 || c >= step_of(fld) - 1)) { fold(fld); ++fld; continue; }
+        // ---- publish the summary of the next finished block (never waits for a decision on itself)
+        if (pub < n_c && pub - fld < NP) {
+          const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
+          const uint32_t par = (pub / NP) & 1;
+          if (!pub_ready) pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
           const int t = step_of(pub);
-          const int slot_i = (t - 1) % M;
-          bool dead = false;                                  // mailbox slot free: step t - M has been scanned
-          while (true) {
-            const int cc = ld_ctrl_relaxed(a_ctrl);
-            if (cc < 0) { dead = true; break; }
-            if (cc >= t - M) break;
-          }
-          if (!dead) {
+          if (pub_ready && c >= 0 && c >= t - M) {            // mailbox slot free: step t - M has been scanned
+            const int slot_i = (t - 1) & (M - 1);
             tc_fence_after();
             float pv[G];
             tmem_ld<G>(tmem_PV + tlane + (pub & (NP - 1)) * kUmmaN, pv);
             tmem_ld_wait();
-            const IterSlot& sl = slots[pub & (NP - 1)];
+            const IterSlot& sl = slots[pub & (kIterSlots - 1)];
             const uint32_t row0 = mapa(sbase + sm.mbox + static_cast<uint32_t>(slot_i) * kSummaryBytes, 0);
             const uint32_t mb = mapa(bar(sm.mbox0 + slot_i), 0);
             if (MODE == 2 || (d & 3) == 0) {
@@ -456,100 +528,58 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
             if (d == 1) {
               float ml[2 * G];
 #pragma unroll
-              for (int h = 0; h < G; ++h) { ml[h] = sl.mref[h]; ml[G + h] = sl.lsum[0][h] + sl.lsum[1][h]; }
+              for (int h = 0; h < G; ++h) { ml[h] = sl.mref[h]; ml[G + h] = sl.lsum[h]; }
               st_async_vec<G>(row0, ml, mb);
               st_async_vec<G>(row0 + G * 4u, ml + G, mb);
             }
+            ++pub; pub_ready = false;
           }
-          ++pub;
-          continue;
         }
-        if (fld >= pub) continue;
-        if (!(c < 0 || c >= step_of(fld) - 1)) continue;      // decision for the steps before it not known yet
-      } else {
-        if (!mbar_try_wait(bar(sm.pvfull0 + (fld & (NP - 1))), (fld / NP) & 1)) continue;
       }
-      // ---- fold block `fld` into its stream: it is part of the result (step <= t*)
-      tc_fence_after();
-      float pv[G];
-      tmem_ld<G>(tmem_PV + tlane + (fld & (NP - 1)) * kUmmaN, pv);
-      tmem_ld_wait();
-      const IterSlot& sl = slots[fld & (NP - 1)];
-      const bool odd = fld & 1;
-#pragma unroll
-      for (int h = 0; h < G; ++h) {
-        const float a = sl.alpha[h], lb = sl.lsum[0][h] + sl.lsum[1][h], mr = sl.mref[h];
-        const float an = fmaf(a, odd ? acc1[h] : acc0[h], pv[h]);
-        const float ln = fmaf(a, odd ? l1[h] : l0[h], lb);
-        if (odd) { acc1[h] = an; l1[h] = ln; m1[h] = mr; } else { acc0[h] = an; l0[h] = ln; m0[h] = mr; }
-      }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.pvfree0 + (fld & (NP - 1))));
-      ++fld;
     }
   } else if (ART && warp == kWarpScan && rank == 0) {
     // ===================================================== A6 + A7 + A9: Algorithm 1 over step summaries
-    constexpr int LPH = 32 / G;                               // lanes per head
-    constexpr int CPL = PW / LPH;                             // probe components per lane
+    using Scan = ScanCore<G, PW>;
+    constexpr int LPH = Scan::LPH, CPL = Scan::CPL;
     const int h = lane / LPH, sub = lane % LPH;
-    float m_run = kNegInf, l_run = 0.f, x[CPL];
+    Scan sc; sc.init();
+    const uint32_t mb_lane = sbase + sm.mbox + h * 4u;         // this lane's head column of a mailbox row block
+    int t_stop = 0;
+    int t = 1;
+    const int mshift = 31 - __clz(M);                         // M is a power of two
+    while (t <= Tn) {
+      const int i0 = t - 1;                                   // 0-based step index of the batch head
+      mbar_wait(bar(sm.mbox0 + (i0 & (M - 1))), (i0 >> mshift) & 1);
+      // how many of the following steps have arrived as well (lane k probes step t + k)
+      int n = 1;
+      {
+        bool ok = false;
+        if (lane >= 1 && lane < kScanBatch && t + lane <= Tn)
+          ok = mbar_test_wait(bar(sm.mbox0 + ((i0 + lane) & (M - 1))), ((i0 + lane) >> mshift) & 1);
+        const uint32_t bits = __ballot_sync(0xffffffffu, ok) | 1u;
+        n = __ffs(~bits) - 1;
+        n = n > kScanBatch ? kScanBatch : n;
+        __syncwarp();                                         // the probing lane's acquire covers the whole warp
+      }
+      const int fired = sc.batch(n, lane, p.tau, p.phi, p.patience,
+        [&](int k, bool live, float& mt, float& lt) {
+          const uint32_t a = mb_lane + static_cast<uint32_t>((i0 + k) & (M - 1)) * kSummaryBytes;
+          const float m_ = lds_f32(a), l_ = lds_f32(a + G * 4u);     // a slot that is not part of the batch
+          mt = live ? m_ : kNegInf; lt = live ? l_ : 0.f;            // may hold anything: select, never use
+        },
+        [&](int k, bool live, float (&pv)[CPL]) {
+          const uint32_t a = mb_lane + static_cast<uint32_t>((i0 + k) & (M - 1)) * kSummaryBytes + (2 + sub) * G * 4u;
 #pragma unroll
-    for (int j = 0; j < CPL; ++j) x[j] = 0.f;                 // x^(0) = 0 (Alg. 1 l.1)
-    int cnt = 0, t_stop = 0;                                  // c^(0) = 0 (l.2)
-    int slot_i = 0; uint32_t mph = 0;                         // (t - 1) % M and ((t - 1) / M) & 1
-    for (int t = 1; t <= Tn; ++t) {
-      mbar_wait(bar(sm.mbox0 + slot_i), mph);
-      const float* mb = mbox + static_cast<size_t>(slot_i) * (2 + PW) * G;
-      const float mt = mb[h], lt = mb[G + h];
-      float pv[CPL];
-#pragma unroll
-      for (int j = 0; j < CPL; ++j) pv[j] = mb[(2 + sub + LPH * j) * G + h];
+          for (int j = 0; j < CPL; ++j) { const float v = lds_f32(a + LPH * j * G * 4u); pv[j] = live ? v : 0.f; }
+        });
       __syncwarp();
-      if (lane == 0 && t + M <= Tn) mbar_arrive_expect_tx(bar(sm.mbox0 + slot_i), kSummaryBytes);   // re-arm for step t + M
-      // streaming update in recurrence form: x^(t) - x^(t-1) = (l_t / A_t) P(u^(t) - o^(t-1))
-      // (PAPER.md:320, :361), with l_t u^(t) = P~V_t and everything relative to the running max.
-      float sdd = 0.f, sad = 0.f, saa = 0.f, sbb = 0.f;
-      if (mt != kNegInf) {                                    // a step with no valid token changes nothing (R8)
-        const float mn = fmaxf(m_run, mt);
-        const float al = fast_exp2(m_run - mn), be = fast_exp2(mt - mn);
-        const float l_new = fmaf(al, l_run, be * lt);
-        const float r = (l_new > 0.f) ? be / l_new : 0.f;
-#pragma unroll
-        for (int j = 0; j < CPL; ++j) {
-          const float dlt = r * fmaf(-lt, x[j], pv[j]);
-          const float xn = x[j] + dlt;
-          sdd = fmaf(dlt, dlt, sdd); sad = fmaf(x[j], dlt, sad); saa = fmaf(x[j], x[j], saa); sbb = fmaf(xn, xn, sbb);
-          x[j] = xn;
-        }
-        m_run = mn; l_run = l_new;
-      } else {
-#pragma unroll
-        for (int j = 0; j < CPL; ++j) { saa = fmaf(x[j], x[j], saa); }
-        sbb = saa;
-      }
-#pragma unroll
-      for (int msk = LPH / 2; msk >= 1; msk >>= 1) {
-        sdd += __shfl_xor_sync(0xffffffffu, sdd, msk); sad += __shfl_xor_sync(0xffffffffu, sad, msk);
-        saa += __shfl_xor_sync(0xffffffffu, saa, msk); sbb += __shfl_xor_sync(0xffffffffu, sbb, msk);
-      }
-      // Eq. 2: d_scale = ||dx||; d_direction = 1 - cos(x_new, x_old), evaluated as
-      // (|a|^2 |d|^2 - (a.d)^2) / (|a||b| (|a||b| + a.b)) to avoid the cancellation in 1 - cos.
-      const float d_scale = sqrtf(sdd);
-      float d_dir = 1.f;                                      // zero norm => cos := 0 (R4)
-      if (saa > 0.f && sbb > 0.f) {
-        const float nanb = sqrtf(saa) * sqrtf(sbb);
-        const float ab = saa + sad;
-        if (ab > 0.f) d_dir = fmaxf(fmaf(saa, sdd, -sad * sad), 0.f) / (nanb * (nanb + ab));
-        else d_dir = 1.f - ab / nanb;
-      }
-      const bool stable_h = (d_scale < p.tau) && (d_dir < p.phi);            // strict (R5)
-      const bool stable = __all_sync(0xffffffffu, stable_h);                 // AND over the group's heads (R2)
-      cnt = stable ? cnt + 1 : 0;                                            // Eq. 3
-      const bool fire = cnt >= p.patience;
-      if (lane < C) st_cluster_relaxed_s32(mapa(a_ctrl, lane), fire ? -t : t);
-      if (fire) { t_stop = t; break; }
-      if (++slot_i == M) { slot_i = 0; mph ^= 1u; }
+      if (fired < 0 && lane < n && t + lane + M <= Tn)        // re-arm the consumed slots for steps t + k + M
+        mbar_arrive_expect_tx(bar(sm.mbox0 + ((i0 + lane) & (M - 1))), kSummaryBytes);
+      __syncwarp();
+      const int t_last = fired >= 0 ? t + fired : t + n - 1;
+      if (lane < C) st_cluster_relaxed_s32(mapa(a_ctrl, lane), fired >= 0 ? -t_last : t_last);
+      if (fired >= 0) { t_stop = t_last; break; }
+      t += n;
     }
     if (lane == 0) p.stop_block[group] = t_stop ? t_stop : Tn;               // t* (R9)
   }
@@ -560,13 +590,11 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   float* cta = reinterpret_cast<float*>(smem + sm.ring);
   float* cta_m = reinterpret_cast<float*>(smem + sm.misc + kCtaM);
   float* cta_l = reinterpret_cast<float*>(smem + sm.misc + kCtaL);
-  if (warp >= kWarpFold0) {
+  if (warp < kWarpFold0 + 4) {
 #pragma unroll
-    for (int h = 0; h < G; ++h) {                             // the CTA's two streams -> one partial state
-      const float mx = fmaxf(m0[h], m1[h]);
-      const float f0 = (m0[h] == kNegInf) ? 0.f : fast_exp2(m0[h] - mx), f1 = (m1[h] == kNegInf) ? 0.f : fast_exp2(m1[h] - mx);
-      cta[h * kD + d] = fmaf(f0, acc0[h], f1 * acc1[h]);
-      if (d == 0) { cta_m[h] = mx; cta_l[h] = fmaf(f0, l0[h], f1 * l1[h]); }
+    for (int h = 0; h < G; ++h) {
+      cta[h * kD + d] = acc[h];
+      if (d == 0) { cta_m[h] = m_tot[h]; cta_l[h] = l_tot[h]; }
     }
   }
   cluster_sync_all();
@@ -594,7 +622,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     }
   }
   cluster_sync_all();                                         // peers' shared memory stays alive until read
-  if (warp == kWarpTmem) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
+  if (warp == kWarpMmaPV) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
 }
 
 }  // namespace tc

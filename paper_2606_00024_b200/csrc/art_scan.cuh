@@ -1,0 +1,149 @@
+// The sequential part of ART: Algorithm 1's criterion and patience counter (PAPER.md:101-133,
+// Eq. 2, Eq. 3) replayed by ONE warp of the cluster leader over the per-step
+// summaries (m_t = reference exponent, l_t = block sum, P~V_t at the probe coordinates).
+//
+// The loop over steps is inherently serial (x^(t) depends on x^(t-1)), so its cost per step bounds the
+// rate at which a group can stream KV blocks.  Only the short recurrence
+//     x^(t) = x^(t-1) + (l_t / A_t) (u^(t)[idx] - x^(t-1))
+// is carried from step to step; everything else (norms, cross-lane sums, sqrt, divide, compare) is
+// independent per step.  The warp therefore takes a BATCH of up to kScanBatch consecutive steps whose
+// summaries have arrived, runs the recurrence over them back to back, reduces the 4 x batch partial sums
+// with one transposing butterfly (each lane ends up owning one step), evaluates Eq. 2 for all steps of
+// the batch in parallel lanes and then walks the patience counter.  The arithmetic per step is exactly
+// the sequential algorithm's; a batch of one is the plain loop.
+#pragma once
+#include "art_common.cuh"
+
+namespace art {
+
+constexpr int kScanBatch = 8;
+
+// Lane layout: the warp's 32 lanes are split into G groups of LPH = 32 / G lanes, one group per head of
+// the query group; lane `sub` of a group owns probe components sub, sub + LPH, ...  (CPL of them).
+template <int G, int PW>
+struct ScanCore {
+  static constexpr int LPH = 32 / G;
+  static constexpr int CPL = PW / LPH;
+  static constexpr int NTR = (LPH >= 8) ? 3 : 2;          // transposing rounds of the butterfly (LPH >= 4)
+  static constexpr int KH = kScanBatch >> NTR;            // steps a lane owns after the reduction (1 or 2)
+  static_assert(G == 1 || G == 2 || G == 4 || G == 8, "group size");
+  static_assert(PW % LPH == 0, "probe width must split over the lanes of a head");
+
+  float m_run, l_run;       // running reference exponent (log2 domain) and A_t relative to it
+  float x[CPL];             // probe of the normalised output, x^(t)
+  int cnt;                  // c^(t)
+
+  __device__ __forceinline__ void init() {
+    m_run = kNegInf; l_run = 0.f; cnt = 0;                // c^(0) = 0 (Alg. 1 l.2)
+#pragma unroll
+    for (int j = 0; j < CPL; ++j) x[j] = 0.f;             // x^(0) = 0 (Alg. 1 l.1)
+  }
+
+  // Sums s[k][q] over the LPH lanes of each head.  Afterwards s[j][q], j < KH, holds the complete sums of
+  // step owned_step(lane) + j.
+  static __device__ __forceinline__ void reduce(float (&s)[kScanBatch][3], int lane) {
+    int cntk = kScanBatch;
+#pragma unroll
+    for (int m = LPH / 2; m >= 1; m >>= 1) {
+      if (cntk > KH) {                                     // transposing round: halve the number of steps held
+        const int half = cntk / 2;
+        const bool up = (lane & m) != 0;
+#pragma unroll
+        for (int i = 0; i < half; ++i)
+#pragma unroll
+          for (int q = 0; q < 3; ++q) {
+            const float keep = up ? s[i + half][q] : s[i][q];
+            const float send = up ? s[i][q] : s[i + half][q];
+            s[i][q] = keep + __shfl_xor_sync(0xffffffffu, send, m);
+          }
+        cntk = half;
+      } else {
+#pragma unroll
+        for (int i = 0; i < KH; ++i)
+#pragma unroll
+          for (int q = 0; q < 3; ++q) s[i][q] += __shfl_xor_sync(0xffffffffu, s[i][q], m);
+      }
+    }
+  }
+  // lane (within its head's LPH lanes) that owns step k after reduce(), and the slot j it sits in
+  static __host__ __device__ constexpr int owner_sub(int k) { return LPH == 4 ? (k >> 1) : k * (LPH / 8); }
+  static __host__ __device__ constexpr int owner_slot(int k) { return LPH == 4 ? (k & 1) : 0; }
+
+  static __device__ __forceinline__ float sqrt_approx(float v) {
+    float r; asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(v)); return r;
+  }
+  // Eq. 2 for one head from the complete sums |dx|^2, x_old.dx, |x_old|^2: d_scale = ||dx||,
+  // d_direction = 1 - cos(x_new, x_old) evaluated as (|a|^2 |d|^2 - (a.d)^2) / (|a||b| (|a||b| + a.b)), which
+  // avoids the cancellation in 1 - cos; the quotient is compared as num < phi * den.  |b|^2 = |a|^2 + 2 a.d +
+  // |d|^2.  Zero norm => cos := 0 (R4); strict '<' (R5).
+  static __device__ __forceinline__ bool stable_head(const float (&s)[3], float tau, float phi) {
+    const float sdd = s[0], sad = s[1], saa = s[2];
+    const float sbb = fmaf(2.f, sad, saa) + sdd;
+    const bool scale_ok = sqrt_approx(sdd) < tau;
+    bool dir_ok = 1.f < phi;
+    if (saa > 0.f && sbb > 0.f) {
+      const float nanb = sqrt_approx(saa) * sqrt_approx(sbb);
+      const float ab = saa + sad;
+      if (ab > 0.f) dir_ok = fmaxf(fmaf(saa, sdd, -sad * sad), 0.f) < phi * (nanb * (nanb + ab));
+      else dir_ok = (1.f - __fdividef(ab, nanb)) < phi;
+    }
+    return scale_ok && dir_ok;
+  }
+
+  // Processes n (1..kScanBatch) consecutive steps.  load_ml(k, mt, lt) / load_pv(k, pv) fetch the summary of
+  // the k-th step of the batch for this lane's head / probe components; they are called for every k <
+  // kScanBatch with `k < n` as a predicate (the code is branch-free so that the loads of all steps and the
+  // independent parts of the arithmetic overlap; a missing step is an empty one and leaves the state as it is).
+  // Returns the 0-based index within the batch of the step at which the criterion fired (c >= patience,
+  // PAPER.md:157), or -1.
+  template <typename LoadML, typename LoadPV>
+  __device__ __forceinline__ int batch(int n, int lane, float tau, float phi, int patience, LoadML&& load_ml, LoadPV&& load_pv) {
+    // ---- the scalar chain: reference exponent and A_t, r_t = 2^(m_t - m) / A_t
+    float lt[kScanBatch], r[kScanBatch];
+#pragma unroll
+    for (int k = 0; k < kScanBatch; ++k) {
+      float mt;
+      load_ml(k, k < n, mt, lt[k]);                        // (-inf, 0) when the predicate is false
+      const float mn = fmaxf(m_run, mt);
+      const float al = (m_run == mn) ? 1.f : fast_exp2(m_run - mn);
+      const float be = (mt == kNegInf) ? 0.f : fast_exp2(mt - mn);   // a step with no valid token changes nothing (R8)
+      const float l_new = fmaf(al, l_run, be * lt[k]);
+      r[k] = (l_new > 0.f) ? __fdividef(be, l_new) : 0.f;
+      m_run = mn; l_run = l_new;
+    }
+    // ---- the recurrence x^(t) = x^(t-1) + r_t (P~V_t - l_t x^(t-1))   (l_t u^(t) = P~V_t)
+    float s[kScanBatch][3];
+#pragma unroll
+    for (int k = 0; k < kScanBatch; ++k) {
+      float pv[CPL];
+      load_pv(k, k < n, pv);                               // zeros when the predicate is false
+      float sdd = 0.f, sad = 0.f, saa = 0.f;
+#pragma unroll
+      for (int j = 0; j < CPL; ++j) {
+        const float dlt = r[k] * fmaf(-lt[k], x[j], pv[j]);
+        sdd = fmaf(dlt, dlt, sdd); sad = fmaf(x[j], dlt, sad); saa = fmaf(x[j], x[j], saa);
+        x[j] += dlt;
+      }
+      s[k][0] = sdd; s[k][1] = sad; s[k][2] = saa;
+    }
+    reduce(s, lane);
+    uint32_t votes[KH];
+#pragma unroll
+    for (int j = 0; j < KH; ++j) votes[j] = __ballot_sync(0xffffffffu, stable_head(s[j], tau, phi));
+    int fired = -1;
+#pragma unroll
+    for (int k = 0; k < kScanBatch; ++k) {
+      uint32_t need = 0;                                   // the lanes (one per head) that own step k
+#pragma unroll
+      for (int h = 0; h < G; ++h) need |= 1u << (h * LPH + owner_sub(k));
+      const bool stable = (votes[owner_slot(k)] & need) == need;     // AND over the group's heads (R2)
+      const int c_new = stable ? cnt + 1 : 0;              // Eq. 3
+      const bool live = (k < n) && (fired < 0);
+      cnt = live ? c_new : cnt;
+      fired = (live && c_new >= patience) ? k : fired;
+    }
+    return fired;
+  }
+};
+
+}  // namespace art

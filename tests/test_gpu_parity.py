@@ -81,6 +81,14 @@ def test_small_configs_firing(index, sub, split):
     assert rep.mean_stop_frac <= 1.0 and (loaded.cpu() >= stop.cpu()).all()
 
 
+@pytest.mark.parametrize("split", [3, 5, 7, 13, 16])
+def test_any_cluster_size_bf16(split):
+    """The tensor-core kernel deals steps round-robin over ANY cluster size; the result is the sequential one."""
+    w = small(1, recency_decay=(0.2, 1.0))
+    check(w, split=split, tau=1e-3, expect_fired=True)
+    check(w, art_on=False, split=split)
+
+
 @pytest.mark.parametrize("layout", [gen.LAYOUT_HND, gen.LAYOUT_NHD])
 def test_layouts_agree(layout):
     w = small(3, sub="a", layout=layout, recency_decay=(0.2, 1.0))
@@ -177,7 +185,7 @@ def test_error_codes_on_device():
     with pytest.raises(a.ArtError) as e:
         a.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table, None, w.seq_lens, out, stop)
     assert e.value.status == -2
-    assert a.art_query_split(a.make_desc(w), True) in (1, 2, 4, 8, 16)
+    assert 1 <= a.art_query_split(a.make_desc(w), True) <= 16
 
 
 def test_host_entry_point():
