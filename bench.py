@@ -42,12 +42,15 @@ def peaks():
 
 
 def committed_traffic():
-    """dram bytes per launch of the dominant kernel from the committed ncu capture, if any."""
-    path = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes per launch of the dominant kernel from the committed ncu capture (profiles/traffic.csv)."""
+    path = os.path.join(ROOT, "profiles", "traffic.csv")
+    out = {}
     if os.path.exists(path):
+        import csv
         with open(path) as f:
-            return json.load(f)
-    return {}
+            for row in csv.DictReader(f):
+                out[row["key"]] = int(row["bytes_per_launch"])
+    return out
 
 
 class ClockSampler:

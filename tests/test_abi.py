@@ -64,7 +64,8 @@ def test_argument_validation_happens_before_cuda(art):
     assert _call_off(art, good_desc(art, dtype=5)) == -3
     assert _call_off(art, good_desc(art, policy=2)) == -1                    # LIST without a list
     assert _call_off(art, good_desc(art, policy=1, sink_tokens=-1)) == -2
-    assert _call_off(art, good_desc(art, split=3)) == -2
+    assert _call_off(art, good_desc(art, split=17)) == -2                    # cluster size > 16
+    assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=3)) == -2   # fp32 path: power of two
     assert _call_off(art, good_desc(art), k=33) == -4                        # ART_ERR_ALIGN
     lib = art.load_library()
     th = art.ArtThresholds(tau=1e-5, phi=1e-3, patience=0, probe_dim=32)
