@@ -134,6 +134,25 @@ def time_loop(fn, steps: int, warmup: int, barrier=None):
     return e0.elapsed_time(e1)            # ms for K steps
 
 
+def rank_seed(rank: int) -> int:
+    """Every rank draws its own configs[1]-shaped batch: the path shards by sequence, no exchange."""
+    from workloads import generators as gen
+    return gen.SEED_BASE + 1000 + 17 * rank
+
+
+def reduce_over_ranks(ms: float, toks: float, device="cpu"):
+    """Whole-job numbers: MAX over ranks of the timed region, SUM over ranks of the units processed.
+    Works with any initialised process group (nccl on the GPU box, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    tk = torch.tensor([float(toks)], dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tk, op=dist.ReduceOp.SUM)
+    return float(t), float(tk)
+
+
 def make_runner(art, w, *, art_on: bool, split: int = 0, **th):
     """Pre-marshalled call (descriptors and outputs allocated once); returns (fn, out, stop, loaded)."""
     import torch
@@ -303,8 +322,8 @@ def main():
     dev = torch.device("cuda", local)
 
     # configs[1]; every rank its own batch (seed offset), no exchange between ranks
-    w = gen.config(1, device=dev, seed=gen.SEED_BASE + 1000 + 17 * rank)
-    wR = gen.config(1, device=dev, variant="R", seed=gen.SEED_BASE + 1000 + 17 * rank)
+    w = gen.config(1, device=dev, seed=rank_seed(rank))
+    wR = gen.config(1, device=dev, variant="R", seed=rank_seed(rank))
     torch.cuda.synchronize()
     toks = eligible_tokens(w)
     peak, which = peaks()
@@ -324,12 +343,7 @@ def main():
     with ClockSampler(local) as cs:
         ms = time_loop(fn, args.steps, args.warmup, barrier)
     clocks = cs.summary()
-    t = torch.tensor([ms], dtype=torch.float64, device=dev)
-    tk = torch.tensor([float(toks)], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tk, op=dist.ReduceOp.SUM)
-    ms_max, toks_all = float(t), float(tk)
+    ms_max, toks_all = reduce_over_ranks(ms, toks, dev)
     ms_per_step = ms_max / args.steps
     value = toks_all / (ms_per_step * 1e-3)
     processed, ld = int(stop.sum()), int(loaded.sum())
@@ -345,10 +359,8 @@ def main():
     for _ in range(args.steps):
         hfn()                                  # synchronises the stream itself
     e2e_ms = (time.perf_counter() - t0) * 1e3
-    te = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_value = toks_all / (float(te) / args.steps * 1e-3)
+    e2e_max, _ = reduce_over_ranks(e2e_ms, 0.0, dev)
+    e2e_value = toks_all / (e2e_max / args.steps * 1e-3)
 
     # ---- context numbers (outside the contract's timed region): ART-off, p = inf, variant R
     off = measure(art, w, args.steps, args.warmup, barrier, art_on=False)
