@@ -108,10 +108,27 @@ def art_query_split(desc: ArtDesc, art_on: bool = True) -> int:
     return int(load_library().art_query_split(C.byref(desc), int(bool(art_on))))
 
 
+_ws_cache = {}
+
+
+def _workspace_for(desc: ArtDesc, device) -> torch.Tensor:
+    """Device scratch of art_workspace_bytes(desc), cached per device (grown on demand).  The library never
+    allocates; the caller (here: the binding, with torch) owns the memory."""
+    need = max(art_workspace_bytes(desc), 256)
+    key = (device.type, device.index)
+    ws = _ws_cache.get(key)
+    if ws is None or ws.numel() < need:
+        ws = torch.empty(need, dtype=torch.uint8, device=device)
+        _ws_cache[key] = ws
+    return ws
+
+
 def art_decode_attention(desc, q, k_cache, v_cache, block_table, eligible_blocks, seq_lens, thresholds,
                          out, stop_block, workspace=None, stream=None) -> None:
     """ART-on.  All tensors are CUDA tensors except desc/thresholds (ctypes structs)."""
-    ws_ptr, ws_bytes = (_ptr(workspace), workspace.numel() * workspace.element_size()) if workspace is not None else (None, 0)
+    if workspace is None:
+        workspace = _workspace_for(desc, q.device)
+    ws_ptr, ws_bytes = (_ptr(workspace), workspace.numel() * workspace.element_size())
     rc = load_library().art_decode_attention(
         C.byref(desc), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_table), _ptr(eligible_blocks),
         _ptr(seq_lens), C.byref(thresholds), _ptr(out), _ptr(stop_block), ws_ptr, ws_bytes, _stream_ptr(stream))
@@ -122,7 +139,9 @@ def art_decode_attention(desc, q, k_cache, v_cache, block_table, eligible_blocks
 def art_decode_attention_off(desc, q, k_cache, v_cache, block_table, eligible_blocks, seq_lens,
                              out, stop_block, workspace=None, stream=None) -> None:
     """ART-off (same kernel, detector compiled out)."""
-    ws_ptr, ws_bytes = (_ptr(workspace), workspace.numel() * workspace.element_size()) if workspace is not None else (None, 0)
+    if workspace is None:
+        workspace = _workspace_for(desc, q.device)
+    ws_ptr, ws_bytes = (_ptr(workspace), workspace.numel() * workspace.element_size())
     rc = load_library().art_decode_attention_off(
         C.byref(desc), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_table), _ptr(eligible_blocks),
         _ptr(seq_lens), _ptr(out), _ptr(stop_block), ws_ptr, ws_bytes, _stream_ptr(stream))

@@ -24,7 +24,8 @@ def needs_build() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or needs_build():
-        cmd = [NVCC] + FLAGS + (["-Xptxas", "-v"] if verbose else []) + SRC + ["-o", LIB]
+        extra = os.environ.get("ART_NVCC_FLAGS", "").split()      # e.g. -DART_TRACE for a debugging build
+        cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + SRC + ["-o", LIB]
         subprocess.run(cmd, check=True)
     return LIB
 

@@ -11,6 +11,7 @@
 #include <utility>
 #include "art_decode_simt.cuh"
 #include "art_decode_tc.cuh"
+#include "art_decode_ws_kernel.cuh"
 
 namespace art {
 
@@ -250,19 +251,62 @@ static int choose_split(const art_desc_t* d, int mode, int* C_out) {
   return ART_OK;
 }
 
+
+// ---- dynamically scheduled kernel (art_decode_ws_kernel.cuh): launch plan
+struct WsPlan { int stages, ms, per_sm; uint32_t smem; };
+static WsPlan plan_ws(int G, int PW, bool art) {
+  WsPlan pl;
+  pl.per_sm = 2; pl.stages = 3; pl.ms = art ? 16 : 0;      // staging window: a power of two, at most 16
+  auto total = [&]() { return ws::make_smem_map_w(G, PW, pl.stages, pl.ms, art).total; };
+  if (total() <= kSmemTwoPerSm) { pl.smem = total(); return pl; }
+  // does not fit twice: one CTA per SM with a deeper ring and a full staging window
+  pl.per_sm = 1; pl.stages = tc::kMaxStages; pl.ms = art ? 16 : 0;
+  while (pl.stages > 2 && total() > static_cast<uint32_t>(kMaxSmem)) --pl.stages;
+  pl.smem = total();
+  return pl;
+}
+
+static int sm_count() {
+  int dev = 0, n = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    cudaGetLastError(); return 0;
+  }
+  return n;
+}
+
+// workspace the dynamically scheduled kernel needs (worst case over the probe widths)
+static size_t ws_bytes_for(const art_desc_t* d) {
+  if (d->dtype != ART_DTYPE_BF16 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads) return 0;
+  const int G = d->num_q_heads / d->num_kv_heads;
+  return ws::make_ws_layout(d->batch * d->num_kv_heads, G, d->head_dim, true).total;
+}
+
+template <typename Kern>
+static cudaError_t launch_ws(Kern kern, int grid, uint32_t smem_bytes, cudaStream_t stream, const Params& p,
+                             const ws::WsView& v, const CUtensorMap& tmK, const CUtensorMap& tmV) {
+  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes));
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, static_cast<int>(cudaSharedmemCarveoutMaxShared));
+  if (e != cudaSuccess) return e;
+  kern<<<grid, tc::kThreads, smem_bytes, stream>>>(p, v, tmK, tmV);
+  return cudaGetLastError();
+}
+
 static int run(const art_desc_t* d, const void* q, const void* k, const void* v, const int32_t* bt,
                const int32_t* elig, const int32_t* elig_counts, const int32_t* sl, const art_thresholds_t* th,
-               float* out, int32_t* stop, int32_t* blocks_loaded, cudaStream_t stream) {
+               float* out, int32_t* stop, int32_t* blocks_loaded, void* workspace, size_t workspace_bytes,
+               cudaStream_t stream) {
   const int groups = d->batch * d->num_kv_heads;
   if (groups == 0) return ART_OK;
   const int G = d->num_q_heads / d->num_kv_heads;
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
+  const bool dynamic = tensor_core && d->split == 0;        // persistent grid, steps claimed at run time
   int C = 1;
-  int rc = choose_split(d, mode, &C);
+  int rc = dynamic ? ART_OK : choose_split(d, mode, &C);
   if (rc != ART_OK) return rc;
-  const LaunchPlan pl = plan_for(tensor_core, G, PW, mode != 0, C);
+  const LaunchPlan pl = dynamic ? LaunchPlan{1, 0, 0, 0u} : plan_for(tensor_core, G, PW, mode != 0, C);
 
   Params p = {};
   p.q = q; p.k = static_cast<const uint8_t*>(k); p.v = static_cast<const uint8_t*>(v);
@@ -283,7 +327,24 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   p.stages = pl.stages; p.mbox_slots = pl.mslots;
 
   cudaError_t e;
-  if (tensor_core) {
+  if (dynamic) {
+    ws::WsLayout lay = ws::make_ws_layout(groups, G, PW, mode != 0);
+    if (!workspace || workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return ART_ERR_WORKSPACE;
+    lay.v.base = static_cast<uint8_t*>(workspace);
+    const WsPlan wp = plan_ws(G, PW, mode != 0);
+    p.stages = wp.stages; p.mbox_slots = wp.ms;
+    const int sms = sm_count();
+    if (sms <= 0) return ART_ERR_CUDA;
+    CUtensorMap tmK, tmV;
+    if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
+      return ART_ERR_CUDA;
+    if (cudaMemsetAsync(workspace, 0, lay.zero_bytes, stream) != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
+    if (blocks_loaded && cudaMemsetAsync(blocks_loaded, 0, sizeof(int32_t) * groups, stream) != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
+    e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
+      return static_cast<int>(launch_ws(ws::art_decode_ws_kernel<decltype(gg)::value, decltype(m)::value>,
+                                        sms * wp.per_sm, wp.smem, stream, p, lay.v, tmK, tmV));
+    }));
+  } else if (tensor_core) {
     CUtensorMap tmK, tmV;
     if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
       return ART_ERR_CUDA;
@@ -311,29 +372,29 @@ int art_decode_attention(const art_desc_t* desc, const void* q, const void* k_ca
                          const int32_t* block_table, const int32_t* eligible_blocks, const int32_t* seq_lens,
                          const art_thresholds_t* thresholds, float* out, int32_t* stop_block,
                          void* workspace, size_t workspace_bytes, void* cuda_stream) {
-  (void)workspace; (void)workspace_bytes;
   if (!thresholds) return ART_ERR_NULL;
   int rc = art::validate(desc, q, k_cache, v_cache, block_table, eligible_blocks, seq_lens, thresholds, out, stop_block, false);
   if (rc != ART_OK) return rc;
   if ((rc = art::check_arch()) != ART_OK) return rc;
   return art::run(desc, q, k_cache, v_cache, block_table, eligible_blocks, desc->eligible_counts, seq_lens,
-                  thresholds, out, stop_block, desc->blocks_loaded, static_cast<cudaStream_t>(cuda_stream));
+                  thresholds, out, stop_block, desc->blocks_loaded, workspace, workspace_bytes,
+                  static_cast<cudaStream_t>(cuda_stream));
 }
 
 int art_decode_attention_off(const art_desc_t* desc, const void* q, const void* k_cache, const void* v_cache,
                              const int32_t* block_table, const int32_t* eligible_blocks, const int32_t* seq_lens,
                              float* out, int32_t* stop_block, void* workspace, size_t workspace_bytes,
                              void* cuda_stream) {
-  (void)workspace; (void)workspace_bytes;
   int rc = art::validate(desc, q, k_cache, v_cache, block_table, eligible_blocks, seq_lens, nullptr, out, stop_block, false);
   if (rc != ART_OK) return rc;
   if ((rc = art::check_arch()) != ART_OK) return rc;
   return art::run(desc, q, k_cache, v_cache, block_table, eligible_blocks, desc->eligible_counts, seq_lens,
-                  nullptr, out, stop_block, desc->blocks_loaded, static_cast<cudaStream_t>(cuda_stream));
+                  nullptr, out, stop_block, desc->blocks_loaded, workspace, workspace_bytes,
+                  static_cast<cudaStream_t>(cuda_stream));
 }
 
 // device scratch layout of the host variant: q | block_table | seq_lens | eligible | counts | out | stop
-struct HostLayout { size_t q, bt, sl, el, ec, out, stop, total; };
+struct HostLayout { size_t q, bt, sl, el, ec, out, stop, kws, total; };
 static HostLayout host_layout(const art_desc_t* d) {
   auto up = [](size_t x) { return (x + 255) & ~static_cast<size_t>(255); };
   HostLayout h; size_t off = 0;
@@ -346,6 +407,7 @@ static HostLayout host_layout(const art_desc_t* d) {
   h.ec = off; off = up(off + (d->policy == ART_POLICY_LIST ? B * Hkv * 4 : 0));
   h.out = off; off = up(off + B * Hq * D * 4);
   h.stop = off; off = up(off + B * Hkv * 4);
+  h.kws = off; off = up(off + art::ws_bytes_for(d));        // scratch of the dynamically scheduled kernel
   h.total = off;
   return h;
 }
@@ -353,6 +415,7 @@ static HostLayout host_layout(const art_desc_t* d) {
 size_t art_workspace_bytes(const art_desc_t* desc) {
   if (!desc || desc->batch < 0 || desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->head_dim <= 0 ||
       desc->max_blocks_per_seq < 0 || desc->max_eligible < 0) return 0;
+  if (desc->num_q_heads % desc->num_kv_heads) return 0;
   return host_layout(desc).total;
 }
 
@@ -383,7 +446,7 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
   rc = art::run(desc, ws + h.q, k_cache, v_cache, reinterpret_cast<const int32_t*>(ws + h.bt),
                 reinterpret_cast<const int32_t*>(ws + h.el), reinterpret_cast<const int32_t*>(ws + h.ec),
                 reinterpret_cast<const int32_t*>(ws + h.sl), thresholds, reinterpret_cast<float*>(ws + h.out),
-                reinterpret_cast<int32_t*>(ws + h.stop), nullptr, st);
+                reinterpret_cast<int32_t*>(ws + h.stop), nullptr, ws + h.kws, h.total - h.kws, st);
   if (rc != ART_OK) return rc;
   ok &= cudaMemcpyAsync(out_host, ws + h.out, B * Hq * D * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   ok &= cudaMemcpyAsync(stop_block_host, ws + h.stop, B * Hkv * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
@@ -400,6 +463,7 @@ int art_query_split(const art_desc_t* desc, int art_on) {
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;
+  if (desc->dtype == ART_DTYPE_BF16 && desc->split == 0) return 0;   // dynamic scheduler: no fixed cluster
   int C = 1;
   rc = art::choose_split(desc, art_on ? 1 : 0, &C);
   return rc == ART_OK ? C : rc;

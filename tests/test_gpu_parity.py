@@ -185,7 +185,7 @@ def test_error_codes_on_device():
     with pytest.raises(a.ArtError) as e:
         a.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table, None, w.seq_lens, out, stop)
     assert e.value.status == -2
-    assert 1 <= a.art_query_split(a.make_desc(w), True) <= 16
+    assert 0 <= a.art_query_split(a.make_desc(w), True) <= 16      # 0 = dynamic scheduler
 
 
 def test_host_entry_point():
@@ -200,12 +200,15 @@ def test_host_entry_point():
     th = a.ArtThresholds(tau=1e-3, phi=1e-3, patience=5, probe_dim=32)
     a.art_decode_attention_host(desc, w.q.pin_memory(), wc.k_cache, wc.v_cache, w.block_table.pin_memory(),
                                 w.eligible_blocks.pin_memory(), w.seq_lens.pin_memory(), th, out, stop, ws)
+    # stop blocks are bit-deterministic; with the dynamic scheduler the order in which partial states are
+    # merged depends on the run, so outputs agree to fp32 rounding, not bit for bit
+    close = lambda x, y: (x - y).abs().max() <= 1e-5 * y.abs().max()
     o_dev, s_dev, _ = a.run_workload(wc, tau=1e-3)
-    assert torch.equal(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
+    assert close(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
     a.art_decode_attention_host(desc, w.q.pin_memory(), wc.k_cache, wc.v_cache, w.block_table.pin_memory(),
                                 w.eligible_blocks.pin_memory(), w.seq_lens.pin_memory(), None, out, stop, ws)
     o_dev, s_dev, _ = a.run_workload(wc, art=False)
-    assert torch.equal(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
+    assert close(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
 
 
 # ------------------------------------------------------------------ BASELINE-size configs, sampled groups
