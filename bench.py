@@ -262,11 +262,12 @@ def run_report(args):
         w = gen.config(index, sub=sub, variant=variant, device="cuda")
         torch.cuda.synchronize()
         toks = eligible_tokens(w)
-        off = measure(art, w, args.steps, args.warmup, art_on=False)
-        on = measure(art, w, args.steps, args.warmup, art_on=True)
-        pinf = measure(art, w, args.steps, args.warmup, art_on=True, patience=art.ART_PATIENCE_INF)
+        sp = args.split if w.dtype == torch.bfloat16 else 0
+        off = measure(art, w, args.steps, args.warmup, art_on=False, split=sp)
+        on = measure(art, w, args.steps, args.warmup, art_on=True, split=sp)
+        pinf = measure(art, w, args.steps, args.warmup, art_on=True, split=sp, patience=art.ART_PATIENCE_INF)
         total_blocks = off["blocks_processed"]
-        row = {"workload": w.name, "groups": w.batch * w.num_kv_heads, "split_on": art.art_query_split(art.make_desc(w), True),
+        row = {"workload": w.name, "groups": w.batch * w.num_kv_heads, "split_on": art.art_query_split(art.make_desc(w, split=sp), True),
                "eligible_tokens": toks, "blocks_total": total_blocks,
                "off_us": round(off["us_per_step"], 2), "off_gbs": round(off["gbs_processed"], 1),
                "off_frac_of_peak": round(off["gbs_processed"] / peak, 4),
@@ -292,7 +293,7 @@ def main():
     ap.add_argument("--impl", default="art", choices=["art", "reference"])
     ap.add_argument("--report", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--split", type=int, default=0, help="cluster size for --arm (0 = library default)")
+    ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
                     help="time ONLY this arm of configs[1] (short command for ncu captures; prints a small JSON line)")
     args = ap.parse_args()
@@ -367,6 +368,9 @@ def main():
     pinf = measure(art, w, args.steps, args.warmup, barrier, art_on=True, patience=art.ART_PATIENCE_INF)
     r_off = measure(art, wR, args.steps, args.warmup, barrier, art_on=False)
     r_on = measure(art, wR, args.steps, args.warmup, barrier, art_on=True)
+    # the dynamically scheduled kernel (desc.split = ART_SPLIT_DYNAMIC), same two workloads
+    d_on = measure(art, w, args.steps, args.warmup, barrier, art_on=True, split=art.ART_SPLIT_DYNAMIC)
+    dr_on = measure(art, wR, args.steps, args.warmup, barrier, art_on=True, split=art.ART_SPLIT_DYNAMIC)
 
     if rank == 0:
         us = ms / args.steps * 1e3             # this rank's own kernel time per launch
@@ -397,7 +401,11 @@ def main():
                                   "speedup_on_vs_off": r_off["us_per_step"] / r_on["us_per_step"],
                                   "skipped_frac": 1.0 - r_on["blocks_processed"] / max(r_off["blocks_processed"], 1),
                                   "loaded_frac": r_on["blocks_loaded"] / max(r_off["blocks_processed"], 1),
-                                  "on_gbs_loaded": r_on["gbs_loaded"], "on_frac_of_peak_loaded": r_on["gbs_loaded"] / peak}},
+                                  "on_gbs_loaded": r_on["gbs_loaded"], "on_frac_of_peak_loaded": r_on["gbs_loaded"] / peak},
+                    "dynamic_scheduler": {"on_us_per_step": d_on["us_per_step"],
+                                          "variant_R_on_us_per_step": dr_on["us_per_step"],
+                                          "variant_R_speedup_on_vs_off": r_off["us_per_step"] / dr_on["us_per_step"],
+                                          "variant_R_loaded_frac": dr_on["blocks_loaded"] / max(r_off["blocks_processed"], 1)}},
         }
         if world == 1 and not args.no_cpu_baseline:
             dt, ctoks, cores = oracle_sample(w, 16)

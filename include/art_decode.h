@@ -35,6 +35,7 @@ extern "C" {
 
 #define ART_VERSION 100          /* 0.1.0 */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
+#define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent grid, steps claimed at run time (BF16 only) */
 #define ART_PATIENCE_INF 2147483647 /* "p = infinity": detector runs, never fires (App. E) */
 
 /* status codes: 0 = OK, negative = error.  No exceptions, no abort. */
@@ -74,8 +75,10 @@ typedef struct art_desc {
   int32_t max_eligible;        /* row stride of eligible_blocks (LIST) */
   float sm_scale;              /* logit scale; 0 => 1/sqrt(d) (Eq. 1) */
   int32_t split;               /* CTAs (thread-block cluster size) cooperating on one group:
-                                  0 = choose automatically, else 1..16 (a power of two for F32).  Any value
-                                  gives the same stop_block as the sequential algorithm. */
+                                  0 = choose automatically, else 1..16 (a power of two for F32), or
+                                  ART_SPLIT_DYNAMIC: no fixed binding, a persistent grid whose CTAs claim steps
+                                  of whichever group has work left (needs `workspace`).  Any value gives the
+                                  same stop_block as the sequential algorithm. */
   const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
   int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
                                   (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */
@@ -103,7 +106,9 @@ typedef struct art_thresholds {
  *   out             DEVICE float32 [B, Hq, d]    o^(t*) (Alg. 1 l.18)
  *   stop_block      DEVICE int32 [B, Hkv]        t* = number of blocks processed, in [0, T];
  *                                                T if the criterion never fired
- *   workspace       unused by this entry point (may be NULL)
+ *   workspace       DEVICE scratch, 256-B aligned, >= art_workspace_bytes(desc); only read and written when
+ *                   desc->split == ART_SPLIT_DYNAMIC (control blocks, step mailboxes, partial states; the
+ *                   call zeroes what it needs), may be NULL otherwise
  *
  * seq_lens[b] == 0 or an empty list gives a zero output row and stop_block 0.
  * Device-side contents (page ids in range, list entries valid) are not validated.

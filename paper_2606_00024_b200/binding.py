@@ -15,6 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_NAME = "libart_decode.so"
 
 ART_PATIENCE_INF = 2**31 - 1
+ART_SPLIT_DYNAMIC = -1
 ART_DTYPE_F32, ART_DTYPE_BF16 = 0, 1
 ART_LAYOUT_HND, ART_LAYOUT_NHD = 0, 1
 ART_POLICY_DENSE, ART_POLICY_SINK_WINDOW, ART_POLICY_LIST = 0, 1, 2

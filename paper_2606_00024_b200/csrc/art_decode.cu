@@ -137,8 +137,9 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
     if (d->max_eligible < 0) return ART_ERR_SHAPE;
   }
   if (d->policy == ART_POLICY_SINK_WINDOW && (d->sink_tokens < 0 || d->window_tokens < 0)) return ART_ERR_SHAPE;
-  if (d->split < 0 || d->split > 16) return ART_ERR_SHAPE;
-  if (d->dtype == ART_DTYPE_F32 && (d->split & (d->split - 1))) return ART_ERR_SHAPE;
+  if (d->split < ART_SPLIT_DYNAMIC || d->split > 16) return ART_ERR_SHAPE;
+  if (d->split == ART_SPLIT_DYNAMIC && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
+  if (d->dtype == ART_DTYPE_F32 && d->split > 0 && (d->split & (d->split - 1))) return ART_ERR_SHAPE;
   if (!(d->sm_scale >= 0.f) || isinf(d->sm_scale)) return ART_ERR_SHAPE;
   if (th) {
     if (th->patience < 1) return ART_ERR_SHAPE;
@@ -302,7 +303,7 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
-  const bool dynamic = tensor_core && d->split == 0;        // persistent grid, steps claimed at run time
+  const bool dynamic = tensor_core && d->split == ART_SPLIT_DYNAMIC;   // persistent grid, steps claimed at run time
   int C = 1;
   int rc = dynamic ? ART_OK : choose_split(d, mode, &C);
   if (rc != ART_OK) return rc;
@@ -463,7 +464,7 @@ int art_query_split(const art_desc_t* desc, int art_on) {
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;
-  if (desc->dtype == ART_DTYPE_BF16 && desc->split == 0) return 0;   // dynamic scheduler: no fixed cluster
+  if (desc->split == ART_SPLIT_DYNAMIC) return 0;                    // dynamic scheduler: no fixed cluster
   int C = 1;
   rc = art::choose_split(desc, art_on ? 1 : 0, &C);
   return rc == ART_OK ? C : rc;

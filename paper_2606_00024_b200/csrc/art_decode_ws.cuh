@@ -61,6 +61,9 @@ struct WsView {
 };
 
 struct WsLayout { WsView v; size_t total, zero_bytes; };
+// one step summary, padded to the 16-byte granularity of bulk copies
+__host__ __device__ constexpr int probe_off_of(int G) { return (2 * G + 3) & ~3; }   // floats: (m, l) pairs, padded to 16 B
+__host__ __device__ constexpr uint32_t pay_bytes_of(int G, int PW) { return (static_cast<uint32_t>((probe_off_of(G) + PW * G) * 4) + 15u) & ~15u; }
 
 #ifdef ART_TRACE   // debugging aid (never in the shipped build): timestamped events of the first CTAs
 constexpr int kTraceCtas = 8, kTraceRoles = 3, kTraceEvents = 2048;
@@ -105,7 +108,7 @@ inline WsLayout make_ws_layout(int groups, int G, int PW, bool art) {
   v.Wmax = static_cast<uint32_t>(fair < 2 ? 2 : (fair > cap ? cap : fair));
   v.M = groups <= 296 ? 64u : 16u;
   v.mshift = groups <= 296 ? 6u : 4u;
-  v.pay_bytes = static_cast<uint32_t>((2 + PW) * G * 4);
+  v.pay_bytes = pay_bytes_of(G, PW);
   v.part_floats = static_cast<uint32_t>(G * (kD + 2));
   v.base = nullptr;
   size_t off = 64;
@@ -135,7 +138,7 @@ __host__ __device__ inline SmemMapW make_smem_map_w(int G, int PW, int stages, i
   m.items = off; off += kItemRing * static_cast<uint32_t>(sizeof(ItemInfo));
   m.sinfo = off; off += static_cast<uint32_t>(stages) * 8u;
   off = (off + 15u) & ~15u;
-  m.stg = off; off += art ? static_cast<uint32_t>(ms) * G * (2 + PW) * 4u : 0u;   // staged step summaries (cp.async)
+  m.stg = off; off += art ? static_cast<uint32_t>(ms) * pay_bytes_of(G, PW) : 0u;   // staged step summaries (cp.async)
   off = (off + 15u) & ~15u;
   m.bars = off;
   uint32_t n = 0;

@@ -14,8 +14,9 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
   constexpr int PW = (MODE == 2) ? kD : 32;
   constexpr int NP = kPVSlots, NS = kSSlots;
   constexpr int LBO_P = p_lbo(G), PBUF = p_buf_bytes(G);
-  constexpr uint32_t kPayBytes = (2 + PW) * G * 4;            // one step summary: [2 + PW][G] floats
-  constexpr int kPayFloats = (2 + PW) * G;
+  constexpr uint32_t kPayBytes = pay_bytes_of(G, PW);         // one step summary: (2 + PW) G floats, padded to 16 B
+  constexpr int kPayFloats = static_cast<int>(kPayBytes / 4);
+  constexpr int kProbeOff = probe_off_of(G);
 
   extern __shared__ __align__(1024) uint8_t smem[];
   const int S = p.stages, MS = p.mbox_slots;
@@ -482,7 +483,7 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
           if (MODE == 2 || (d & 3) == 0) {
             const int pi = (MODE == 2) ? d : (d >> 2);          // probe coordinate k*(d/32)  (R1)
 #pragma unroll
-            for (int h = 0; h < G; ++h) pay[2 * G + h * PW + pi] = tag_word(pv[h], par);
+            for (int h = 0; h < G; ++h) pay[kProbeOff + h * PW + pi] = tag_word(pv[h], par);
           }
           if (d == 1) {
             const IterSlotW<G>& sl = slots[pub & (kIterSlots - 1)];
@@ -559,7 +560,7 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
 #pragma unroll
             for (int k = 0; k < KC; ++k) {
               ml[k] = lds_v2(sh + (k0 + k) * kPayBytes + h * 8u);
-              lds_vec<CPL>(sh + (k0 + k) * kPayBytes + (2 * G + h * PW + sub * CPL) * 4u, pv[k]);
+              lds_vec<CPL>(sh + (k0 + k) * kPayBytes + (kProbeOff + h * PW + sub * CPL) * 4u, pv[k]);
             }
 #pragma unroll
             for (int k = 0; k < KC; ++k) {
@@ -581,7 +582,7 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
                 mt = (live && ml.x > -1.0e29f) ? ml.x : kNegInf; lt = live ? ml.y : 0.f;
               },
               [&](int k, bool live, float (&pv)[CPL]) {
-                lds_vec<CPL>(s0 + k * kPayBytes + (2 * G + h * PW + sub * CPL) * 4u, pv);
+                lds_vec<CPL>(s0 + k * kPayBytes + (kProbeOff + h * PW + sub * CPL) * 4u, pv);
 #pragma unroll
                 for (int j = 0; j < CPL; ++j) pv[j] = live ? pv[j] : 0.f;
               });

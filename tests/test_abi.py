@@ -65,6 +65,8 @@ def test_argument_validation_happens_before_cuda(art):
     assert _call_off(art, good_desc(art, policy=2)) == -1                    # LIST without a list
     assert _call_off(art, good_desc(art, policy=1, sink_tokens=-1)) == -2
     assert _call_off(art, good_desc(art, split=17)) == -2                    # cluster size > 16
+    assert _call_off(art, good_desc(art, split=-2)) == -2
+    assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=-1)) == -3   # dynamic: bf16 only
     assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=3)) == -2   # fp32 path: power of two
     assert _call_off(art, good_desc(art), k=33) == -4                        # ART_ERR_ALIGN
     lib = art.load_library()

@@ -65,7 +65,7 @@ def small(index, **kw):
 
 
 @pytest.mark.parametrize("index,sub", [(1, "a"), (2, "a"), (3, "a"), (3, "b"), (4, "a")])
-@pytest.mark.parametrize("split", [0, 1, 2, 4])
+@pytest.mark.parametrize("split", [0, 1, 2, 4, -1])
 def test_small_configs_literal_and_off(index, sub, split):
     w = small(index, sub=sub)
     check(w, split=split)                       # paper-default thresholds: never fires on these (F1)
@@ -73,7 +73,7 @@ def test_small_configs_literal_and_off(index, sub, split):
 
 
 @pytest.mark.parametrize("index,sub", [(1, "a"), (2, "a"), (3, "a"), (3, "b"), (4, "a")])
-@pytest.mark.parametrize("split", [1, 2, 4, 8])
+@pytest.mark.parametrize("split", [1, 2, 4, 8, -1])
 def test_small_configs_firing(index, sub, split):
     """Recency decay strong enough that ART fires mid-stream at these short contexts."""
     w = small(index, sub=sub, recency_decay=(0.2, 1.0))
@@ -103,6 +103,31 @@ def test_group_sizes(G, dtype):
                           seq_lens=[1000, 64, 3111], dtype=dtype, recency_decay=(0.3, 1.0))
     check(w, tau=1e-3, split=2, expect_fired=True)
     check(w, art_on=False, split=4)
+
+
+@pytest.mark.parametrize("G", [1, 2, 4, 8])
+def test_dynamic_scheduler_group_sizes_and_edges(G):
+    """split = ART_SPLIT_DYNAMIC: persistent grid, steps claimed at run time; same stop blocks as Algorithm 1."""
+    w = gen.make_workload("dg", seed=15 + G, batch=3, num_q_heads=2 * G, num_kv_heads=2, head_dim=128,
+                          seq_lens=[1000, 64, 3111], dtype=torch.bfloat16, recency_decay=(0.3, 1.0))
+    check(w, tau=1e-3, split=-1, expect_fired=True)
+    check(w, art_on=False, split=-1)
+    check(w, tau=2e-3, probe_dim=0, split=-1)
+    lens = [0, 1, 63, 64, 65, 130]
+    e = gen.make_workload("de", seed=3, batch=6, num_q_heads=2 * G, num_kv_heads=2, head_dim=128, seq_lens=lens)
+    out, stop, _, _ = check(e, split=-1)
+    assert (out[0] == 0).all() and (stop[0] == 0).all()
+    check(e, art_on=False, split=-1)
+
+
+def test_dynamic_scheduler_stop_blocks_equal_cluster_kernel():
+    a = art()
+    w = small(1, recency_decay=(0.2, 1.0)); wc = w.to("cuda")
+    ref_o, ref_s, _ = a.run_workload(wc, tau=1e-3, split=1)
+    for _ in range(3):                          # the schedule differs from run to run, the result must not
+        o, s, _ = a.run_workload(wc, tau=1e-3, split=-1)
+        assert torch.equal(s, ref_s)
+        assert (o - ref_o).abs().max() <= 1e-5 * ref_o.abs().max()
 
 
 def test_full_probe():
@@ -185,7 +210,8 @@ def test_error_codes_on_device():
     with pytest.raises(a.ArtError) as e:
         a.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table, None, w.seq_lens, out, stop)
     assert e.value.status == -2
-    assert 0 <= a.art_query_split(a.make_desc(w), True) <= 16      # 0 = dynamic scheduler
+    assert 1 <= a.art_query_split(a.make_desc(w), True) <= 16
+    assert a.art_query_split(a.make_desc(w, split=-1), True) == 0   # dynamic scheduler: no fixed cluster
 
 
 def test_host_entry_point():
@@ -213,7 +239,7 @@ def test_host_entry_point():
 
 # ------------------------------------------------------------------ BASELINE-size configs, sampled groups
 
-FULL = [(1, "a", ""), (1, "a", "R"), (2, "a", ""), (2, "a", "R"), (3, "a", "R"), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
+FULL = [(1, "a", ""), (1, "a", "R"), (1, "a", "Rdyn"), (4, "a", "Rdyn"), (3, "a", ""), (3, "b", ""), (2, "a", ""), (2, "a", "R"), (3, "a", "R"), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
 
 
 @pytest.mark.parametrize("index,sub,variant", FULL)
@@ -221,13 +247,15 @@ def test_full_size_sampled(index, sub, variant):
     """configs[1..4] at BASELINE.json's sizes, in the launch configuration bench.py times (split = 0,
     auto), ART-on and ART-off; the oracle recomputes sampled groups one by one."""
     a = art()
+    split = -1 if variant.endswith("dyn") else 0
+    variant = variant.replace("dyn", "")
     w = gen.config(index, sub=sub, variant=variant, device="cuda")
     torch.cuda.synchronize()
     rng = np.random.default_rng(index * 10 + len(variant))
     B, Hkv = w.batch, w.num_kv_heads
     groups = sorted({(int(rng.integers(B)), int(rng.integers(Hkv))) for _ in range(5)})
     for art_on in (True, False):
-        out, stop, loaded = a.run_workload(w, art=art_on, want_loaded=True)
+        out, stop, loaded = a.run_workload(w, art=art_on, want_loaded=True, split=split)
         torch.cuda.synchronize()
         assert torch.isfinite(out).all()
         mini = extract_groups(w, groups)
