@@ -50,6 +50,9 @@ constexpr int kPVSlots = 8;                  // unfolded P~V_t results (16 TMEM 
 constexpr int kTmemCols = 256;               // 4 x 32 + 8 x 16; two CTAs share the SM's 512 columns
 constexpr int kIterSlots = 16;               // softmax -> fold hand-over ring; >= kPVSlots + max stages
 constexpr int kMaxStages = 6;
+// P^T (hi, lo) buffers: one per ring stage, except for G = 8 with the detector on, where shared memory only has room for two (block i
+// then uses buffer i & 1, free again once P~V_(i-2) is complete)
+__host__ __device__ constexpr int p_bufs(int G, int stages, bool art32) { return (G == 8 && art32) ? 2 : stages; }
 constexpr int kBoxBytes = 8192;              // one TMA box: 64 rows x 128 bytes
 constexpr int kFront = 12288;                // mapped bytes the S MMA may read below a K tile (3 x 32 rows)
 // Q^T as B operand (K-major, no swizzle): [16 d-chunks of 8][rows][16 B], chunk stride 128 B.  Rows 8-15 of
@@ -78,7 +81,7 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   SmemMap m;
   uint32_t off = 0;
   m.qb = off; off += kQBytes;
-  m.pb = off; off += static_cast<uint32_t>(stages) * 2u * p_buf_bytes(G);
+  m.pb = off; off += static_cast<uint32_t>(p_bufs(G, stages, art && PW == 32)) * 2u * p_buf_bytes(G);
   m.slots = off; off += kIterSlots * static_cast<uint32_t>(sizeof(IterSlot));
   m.sinfo = off; off += static_cast<uint32_t>(stages) * 8u;
   off = (off + 15u) & ~15u;                // mailbox rows are written with 16-byte st.async
@@ -93,14 +96,14 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   m.mbox0 = n; n += art ? mslots : 0;
   m.nbars = n;
   off += n * 8u;
-  m.misc = off; off += 128u;             // ctrl, loaded, tmem_ptr, cta_m[8], cta_l[8]
+  m.misc = off; off += 16u;              // ctrl, loaded, tmem_ptr
   off = (off + 1023u) & ~1023u;
   if (off < static_cast<uint32_t>(kFront)) off = kFront;
   m.ring = off; off += static_cast<uint32_t>(stages) * kStageBytes;
   m.total = off;
   return m;
 }
-constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8, kCtaM = 32, kCtaL = 64;
+constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8;
 
 // ----------------------------------------------------------------------------- tcgen05 / TMA wrappers
 
@@ -223,6 +226,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   constexpr int PW = (MODE == 2) ? kD : 32;          // probe width m
   constexpr int NP = kPVSlots, NS = kSSlots;
   constexpr int LBO_P = p_lbo(G), PBUF = p_buf_bytes(G);
+  constexpr bool kTwoPBufs = (G == 8 && MODE == 1);
   constexpr uint32_t kSummaryBytes = (2 + PW) * G * 4;   // mailbox row block of one step: [2 + PW][G] floats
 
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -272,7 +276,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     }
     if (tid < 64) reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + 16 * kQLbo)[tid] = __float2bfloat16_rn(0.f);
     uint4* pz = reinterpret_cast<uint4*>(smem + sm.pb);        // P^T rows are read before they are first written
-    for (int idx = tid; idx < S * 2 * PBUF / 16; idx += kThreads) pz[idx] = make_uint4(0u, 0u, 0u, 0u);
+    for (int idx = tid; idx < p_bufs(G, S, MODE == 1) * 2 * PBUF / 16; idx += kThreads) pz[idx] = make_uint4(0u, 0u, 0u, 0u);
   }
   fence_proxy_async();          // Q^T written by threads, read by the tensor core
   tc_fence_before();
@@ -389,7 +393,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (i >= NP && !wait_or_stop(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1, t)) break;
         tc_fence_after();
         const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
-        const uint32_t pb = sbase + sm.pb + st * 2 * PBUF;
+        const uint32_t pb = sbase + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF;
 #pragma unroll
         for (int part = 0; part < 2; ++part)                  // p = hi + lo
 #pragma unroll
@@ -419,6 +423,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+      // P^T buffer i & 1 is read by the P.V MMA of block i - 2: wait until that one is complete
+      if (kTwoPBufs && i >= 2 && !wait_or_stop(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1, t)) break;
       const unsigned long long vmask = sinfo[st];             // written before the loads the S MMA waited for
       const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
       float mb[G];
@@ -428,7 +434,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
         mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
       }
-      uint8_t* pb0 = smem + sm.pb + st * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;   // token `lane`, row 0, hi
+      uint8_t* pb0 = smem + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;   // token `lane`, row 0, hi
       float ls[G];
 #pragma unroll
       for (int h = 0; h < G; ++h) {
@@ -588,8 +594,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   tc_fence_before();
   __syncthreads();                                            // ring is free: all loads drained, all MMAs retired
   float* cta = reinterpret_cast<float*>(smem + sm.ring);
-  float* cta_m = reinterpret_cast<float*>(smem + sm.misc + kCtaM);
-  float* cta_l = reinterpret_cast<float*>(smem + sm.misc + kCtaL);
+  float* cta_m = cta + G * kD;
+  float* cta_l = cta_m + G;
   if (warp < kWarpFold0 + 4) {
 #pragma unroll
     for (int h = 0; h < G; ++h) {
