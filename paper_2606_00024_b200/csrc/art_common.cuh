@@ -39,7 +39,39 @@ struct Params {
   float tau, phi;
   int32_t patience;
   int32_t stages, mbox_slots;
+#ifdef ART_TRACE
+  uint8_t* trace;
+#endif
 };
+
+#ifdef ART_TRACE   // debugging aid (never in the shipped build): timestamped events of the first CTAs
+constexpr int kTraceCtas = 8, kTraceRoles = 3, kTraceEvents = 2048;
+__device__ __forceinline__ unsigned long long trace_now() {
+  unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
+}
+struct Tracer {      // roles claim one of kTraceCtas trace slots when they first have something to say
+  uint8_t* region; ulonglong2* buf; int n, role; volatile int* share;
+  __device__ __forceinline__ void init(uint8_t* base, size_t off, int role_, volatile int* share_) {
+    region = base + off; buf = nullptr; n = 0; role = role_; share = share_;
+  }
+  __device__ __forceinline__ void ev(int code, int a, int b) {
+    if (region == nullptr) return;
+    if (!buf) {
+      int slot;
+      if (role == 1) { slot = *share - 1; if (slot < 0) return; }            // fold follows its producer
+      else {
+        if (n < 0) return;
+        slot = atomicAdd(reinterpret_cast<int*>(region) + role, 1);
+        if (role == 0) *share = slot < kTraceCtas ? slot + 1 : 0;
+        if (slot >= kTraceCtas) { n = -1; return; }
+      }
+      if (slot >= kTraceCtas) return;
+      buf = reinterpret_cast<ulonglong2*>(region + 256) + (slot * kTraceRoles + role) * kTraceEvents;
+    }
+    if (n >= 0 && n < kTraceEvents) { buf[n++] = make_ulonglong2(trace_now(), (static_cast<unsigned long long>(code) << 48) | (static_cast<unsigned long long>(a & 0xffffff) << 24) | static_cast<unsigned long long>(b & 0xffffff)); }
+  }
+};
+#endif
 
 // ----------------------------------------------------------------------------- PTX wrappers
 

@@ -38,6 +38,14 @@
 namespace art {
 namespace tc {
 
+#ifdef ART_TRACE
+#define TC_TRACE_INIT(tr, role) Tracer tr; tr.init(p.trace, 0, role, reinterpret_cast<volatile int*>(smem + sm.misc + 12))
+#define TC_TRACE(tr, code, a, b) tr.ev(code, a, b)
+#else
+#define TC_TRACE_INIT(tr, role)
+#define TC_TRACE(tr, code, a, b)
+#endif
+
 constexpr int kThreads = 384;
 // Fold and softmax warps must sit at warp % 4 == TMEM lane quadrant.  The single-thread roles and the scan warp
 // get the highest warp ids: the SM's schedulers favour them, and their latency is what the pipeline feels.
@@ -251,6 +259,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   const int Tn = tr.T;
   const int n_c = (Tn > rank) ? (Tn - rank + C - 1) / C : 0;   // steps owned by this CTA
 
+#ifdef ART_TRACE
+  unsigned long long* cta_times = p.trace ? reinterpret_cast<unsigned long long*>(p.trace + 256 + static_cast<size_t>(kTraceCtas) * kTraceRoles * kTraceEvents * 16) + 4 * blockIdx.x : nullptr;
+  if (tid == 0 && cta_times) cta_times[0] = trace_now();
+#endif
   // ---- one-time setup: barriers, tensor memory, Q^T
   if (tid == 0) {
     for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 32); }
@@ -263,7 +275,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (rank == 0 && s < Tn) mbar_arrive_expect_tx(bar(sm.mbox0 + s), kSummaryBytes);   // armed for steps 1..M
       }
     }
-    st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_loaded, 0);
+    st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_loaded, 0); st_volatile_s32(sbase + sm.misc + 12, 0);
     fence_mbar_init();
   }
   if (warp == kWarpMmaPV) tmem_alloc(a_tmem, kTmemCols);
@@ -307,6 +319,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   if (warp == kWarpProducer) {
     // ===================================================== A1 + A2: resolve blocks, issue TMA loads
     int it_issued = 0, loaded = 0, stage = 0;
+    TC_TRACE_INIT(trc, 0);
     uint32_t ph = 0;                                          // (it / S) & 1
     bool stop = false;
     for (int i0 = 0; i0 < n_c && !stop; i0 += 32) {
@@ -330,6 +343,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (!stop && beyond_stop(t)) stop = true;            // A7: stop issuing prefetch once fired
         if (stop) break;
         if (lane == 0) {
+          TC_TRACE(trc, 1, group, t);
           const uint32_t fb = bar(sm.full0 + stage);
           const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
           sinfo[stage] = mask_k;
@@ -349,6 +363,9 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       }
     }
     if (lane == 0) st_volatile_s32(a_loaded, loaded);
+#ifdef ART_TRACE
+    if (lane == 0 && cta_times) cta_times[2] = trace_now();
+#endif
     // drain: tensor copies still in flight must land before the CTA reuses the ring or exits (H5)
     for (int j = max(0, it_issued - S); j < it_issued; ++j) mbar_wait(bar(sm.full0 + j % S), (j / S) & 1);
   } else if (warp == kWarpMmaS) {
@@ -477,6 +494,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   } else if (warp < kWarpFold0 + 4) {
     // ===================================================== A5 / A6: publish step summaries, merge P~V_t
     const uint32_t tlane = static_cast<uint32_t>(fq * 32) << 16;
+    TC_TRACE_INIT(trf, 1);
     // merge block i (its P~V_t is relative to its own block maximum) into the running state
     auto fold = [&](int i) {
       tc_fence_after();
@@ -498,6 +516,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       tc_fence_before();
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(sm.pvfree0 + (i & (NP - 1))));
+      if (tid == 0) TC_TRACE(trf, 5, i, step_of(i));
     };
     if constexpr (!ART) {
       for (int i = 0; i < n_c; ++i) {
@@ -538,6 +557,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
               st_async_vec<G>(row0, ml, mb);
               st_async_vec<G>(row0 + G * 4u, ml + G, mb);
             }
+            if (tid == 0) TC_TRACE(trf, 4, pub, t);
             ++pub; pub_ready = false;
           }
         }
@@ -549,6 +569,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     constexpr int LPH = Scan::LPH, CPL = Scan::CPL;
     const int h = lane / LPH, sub = lane % LPH;
     Scan sc; sc.init();
+    TC_TRACE_INIT(trs, 2);
     const uint32_t mb_lane = sbase + sm.mbox + h * 4u;         // this lane's head column of a mailbox row block
     int t_stop = 0;
     int t = 1;
@@ -583,6 +604,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         mbar_arrive_expect_tx(bar(sm.mbox0 + ((i0 + lane) & (M - 1))), kSummaryBytes);
       __syncwarp();
       const int t_last = fired >= 0 ? t + fired : t + n - 1;
+      if (lane == 0) TC_TRACE(trs, 8, t, n);
       if (lane < C) st_cluster_relaxed_s32(mapa(a_ctrl, lane), fired >= 0 ? -t_last : t_last);
       if (fired >= 0) { t_stop = t_last; break; }
       t += n;
@@ -629,6 +651,9 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   }
   cluster_sync_all();                                         // peers' shared memory stays alive until read
   if (warp == kWarpMmaPV) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
+#ifdef ART_TRACE
+  if (tid == 0 && cta_times) cta_times[1] = trace_now();
+#endif
 }
 
 }  // namespace tc

@@ -65,32 +65,7 @@ struct WsLayout { WsView v; size_t total, zero_bytes; };
 __host__ __device__ constexpr int probe_off_of(int G) { return (2 * G + 3) & ~3; }   // floats: (m, l) pairs, padded to 16 B
 __host__ __device__ constexpr uint32_t pay_bytes_of(int G, int PW) { return (static_cast<uint32_t>((probe_off_of(G) + PW * G) * 4) + 15u) & ~15u; }
 
-#ifdef ART_TRACE   // debugging aid (never in the shipped build): timestamped events of the first CTAs
-constexpr int kTraceCtas = 8, kTraceRoles = 3, kTraceEvents = 2048;
-__device__ __forceinline__ unsigned long long trace_now() {
-  unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
-}
-struct Tracer {      // roles claim one of kTraceCtas trace slots when they first have something to say
-  uint8_t* region; ulonglong2* buf; int n, role; volatile int* share;
-  __device__ __forceinline__ void init(uint8_t* base, size_t off, int role_, volatile int* share_) {
-    region = base + off; buf = nullptr; n = 0; role = role_; share = share_;
-  }
-  __device__ __forceinline__ void ev(int code, int a, int b) {
-    if (!buf) {
-      int slot;
-      if (role == 1) { slot = *share - 1; if (slot < 0) return; }            // fold follows its producer
-      else {
-        if (n < 0) return;
-        slot = atomicAdd(reinterpret_cast<int*>(region) + role, 1);
-        if (role == 0) *share = slot < kTraceCtas ? slot + 1 : 0;
-        if (slot >= kTraceCtas) { n = -1; return; }
-      }
-      if (slot >= kTraceCtas) return;
-      buf = reinterpret_cast<ulonglong2*>(region + 256) + (slot * kTraceRoles + role) * kTraceEvents;
-    }
-    if (n >= 0 && n < kTraceEvents) { buf[n++] = make_ulonglong2(trace_now(), (static_cast<unsigned long long>(code) << 48) | (static_cast<unsigned long long>(a & 0xffffff) << 24) | static_cast<unsigned long long>(b & 0xffffff)); }
-  }
-};
+#ifdef ART_TRACE
 #define TRACE_INIT(tr, role) Tracer tr; tr.init(w.base, w.off_trace, role, reinterpret_cast<volatile int*>(smem + sm.misc + 16))
 #define TRACE(tr, code, a, b) tr.ev(code, a, b)
 #else
@@ -117,7 +92,7 @@ inline WsLayout make_ws_layout(int groups, int G, int PW, bool art) {
   v.off_pay = off; off = up(off + (art ? static_cast<size_t>(groups) * v.M * v.pay_bytes : 0));
   v.off_trace = off;
 #ifdef ART_TRACE
-  off = up(off + 256 + static_cast<size_t>(kTraceCtas) * kTraceRoles * kTraceEvents * 16);
+  off = up(off + 256 + static_cast<size_t>(kTraceCtas) * kTraceRoles * kTraceEvents * 16 + 1024 * 16);   // + per-CTA (start, end)
 #endif
   l.zero_bytes = off;
   v.off_part = off; off = up(off + static_cast<size_t>(groups) * v.Wmax * v.part_floats * 4);

@@ -40,6 +40,10 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
   auto ctl = [&](int grp) { return ctl_base + grp * kCtlInts; };
   const int M = static_cast<int>(w.M), Wmax = static_cast<int>(w.Wmax);
 
+#ifdef ART_TRACE
+  unsigned long long* cta_times = reinterpret_cast<unsigned long long*>(w.base + w.off_trace + 256 + static_cast<size_t>(kTraceCtas) * kTraceRoles * kTraceEvents * 16) + 2 * blockIdx.x;
+  if (tid == 0) cta_times[0] = trace_now();
+#endif
   // ---- one-time setup
   if (tid == 0) {
     for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 32); }
@@ -624,6 +628,9 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
   tc_fence_before();
   __syncthreads();
   if (warp == kWarpMmaPV) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
+#ifdef ART_TRACE
+  if (tid == 0) cta_times[1] = trace_now();
+#endif
 }
 
 }  // namespace ws
