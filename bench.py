@@ -9,6 +9,7 @@ Hq 32 / Hkv 8, d 128, context 32768, bf16 paged KV, dense policy, paper-default 
     python bench.py [--gpus N] [--steps K] [--warmup W]          # this repo's CUDA path
     python bench.py --impl reference ...                          # the CPU oracle, as it stands
     python bench.py --report                                       # all five configs (+ variants), one JSON line each
+    python bench.py --study                                        # probe-vs-full, ablation, sensitivity
 
 Prints ONE JSON line (rank 0).  `value` is KV tokens/s (sum over sequences of eligible tokens per
 step / step time) with inputs resident in HBM; `e2e` is the same through art_decode_attention_host
@@ -285,6 +286,56 @@ def run_report(args):
         torch.cuda.empty_cache()
 
 
+def run_study(args):
+    """SURVEY 8(f) items 1-2 on the synthetic variant-R workloads: probe (m = 32) vs full-output detector
+    (App. B / Table 4 protocol), the ablation switches of Table 3 and the sensitivity
+    grid of App. F.  Everything runs through the C ABI; one JSON line per row."""
+    import torch
+    from workloads import generators as gen
+    import paper_2606_00024_b200 as art
+    inf = float("inf")
+    for index in (1, 4):
+        w = gen.config(index, variant="R", device="cuda")
+        torch.cuda.synchronize()
+        name = w.name
+        T = measure(art, w, 3, 3, art_on=False)["blocks_processed"] / (w.batch * w.num_kv_heads)
+        o_off, _, _ = art.run_workload(w, art=False)
+
+        def row(kind, **th):
+            m = measure(art, w, args.steps, args.warmup, art_on=True, **th)
+            out, stop, _ = art.run_workload(w, art=True, **th)
+            err = float(((out - o_off).abs().amax(dim=-1) / o_off.abs().amax(dim=-1)).max())
+            return {"study": kind, "workload": name, **{k: (str(v) if v == inf else v) for k, v in th.items()},
+                    "us": round(m["us_per_step"], 1), "mean_stop_frac": round(float(stop.float().mean()) / T, 4),
+                    "fired_frac": round(float((stop.float() < T).float().mean()), 4),
+                    "max_rel_trunc_err_vs_off": err}, stop
+
+        # ---- probe vs full output (the paper's "oracle detector" = P = I)
+        r32, s32 = row("probe_vs_full", probe_dim=32)
+        r0, s0 = row("probe_vs_full", probe_dim=0)
+        d = (s32 - s0).float()
+        cmp = {"study": "probe_vs_full_summary", "workload": name, "groups": int(s32.numel()),
+               "agree_frac": float((d == 0).float().mean()), "probe_earlier_frac(FP)": float((d < 0).float().mean()),
+               "probe_later_frac(FN)": float((d > 0).float().mean()), "mean_abs_delta_blocks": float(d.abs().mean()),
+               "us_probe32": r32["us"], "us_full": r0["us"]}
+        for r in (r32, r0, cmp):
+            print(json.dumps(r), flush=True)
+        # ---- ablation switches (Table 3): each is a threshold setting
+        for label, th in (("default", {}), ("wo_d_scale", {"tau": inf}), ("wo_d_direction", {"phi": inf}),
+                          ("wo_patience", {"patience": 1})):
+            r, _ = row("ablation:" + label, **th)
+            print(json.dumps(r), flush=True)
+        # ---- sensitivity (App. F): one parameter at a time around the defaults
+        for tau in (1e-6, 1e-5, 1e-4):
+            print(json.dumps(row("sensitivity", tau=tau)[0]), flush=True)
+        for phi in (1e-4, 1e-3, 1e-2):
+            print(json.dumps(row("sensitivity", phi=phi)[0]), flush=True)
+        for pt in (1, 2, 5, 10):
+            print(json.dumps(row("sensitivity", patience=pt)[0]), flush=True)
+        del w, o_off
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -292,6 +343,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="art", choices=["art", "reference"])
     ap.add_argument("--report", action="store_true")
+    ap.add_argument("--study", action="store_true", help="probe-vs-full, ablation and sensitivity sweeps (SURVEY 8(f))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
@@ -307,6 +359,9 @@ def main():
         return
     if args.report:
         run_report(args)
+        return
+    if args.study:
+        run_study(args)
         return
 
     import torch
