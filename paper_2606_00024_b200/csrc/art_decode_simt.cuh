@@ -477,7 +477,8 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
         const bool stable = __all_sync(0xffffffffu, stable_h);               // AND over the group's heads (R2)
         cnt = stable ? cnt + 1 : 0;                                          // Eq. 3
         const bool fire = cnt >= p.patience;
-        if (lane < C) st_cluster_release_s32(mapa(a_ctrl, lane), fire ? -t : t);
+        // relaxed is enough: the value depends on this step's mailbox loads, so they have completed
+        if (lane < C) asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(mapa(a_ctrl, lane)), "r"(fire ? -t : t) : "memory");
         if (fire) { t_stop = t; break; }
       }
       if (lane == 0) p.stop_block[group] = t_stop ? t_stop : Tn;             // t* (R9)
