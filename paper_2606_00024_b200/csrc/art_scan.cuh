@@ -24,8 +24,9 @@ template <int G, int PW>
 struct ScanCore {
   static constexpr int LPH = 32 / G;
   static constexpr int CPL = PW / LPH;
-  static constexpr int NTR = (LPH >= 8) ? 3 : 2;          // transposing rounds of the butterfly (LPH >= 4)
-  static constexpr int KH = kScanBatch >> NTR;            // steps a lane owns after the reduction (1 or 2)
+  // steps a lane owns after the reduction of a batch of NB steps (1, or 2 when the head has fewer lanes than NB)
+  template <int NB> static __host__ __device__ constexpr int kh() { return NB > LPH ? NB / LPH : 1; }
+  static constexpr int KH = kh<kScanBatch>();
   static_assert(G == 1 || G == 2 || G == 4 || G == 8, "group size");
   static_assert(PW % LPH == 0, "probe width must split over the lanes of a head");
 
@@ -41,8 +42,10 @@ struct ScanCore {
 
   // Sums s[k][q] over the LPH lanes of each head.  Afterwards s[j][q], j < KH, holds the complete sums of
   // step owned_step(lane) + j.
-  static __device__ __forceinline__ void reduce(float (&s)[kScanBatch][3], int lane) {
-    int cntk = kScanBatch;
+  template <int NB>
+  static __device__ __forceinline__ void reduce(float (&s)[NB][3], int lane) {
+    constexpr int KH = kh<NB>();
+    int cntk = NB;
 #pragma unroll
     for (int m = LPH / 2; m >= 1; m >>= 1) {
       if (cntk > KH) {                                     // transposing round: halve the number of steps held
@@ -66,8 +69,8 @@ struct ScanCore {
     }
   }
   // lane (within its head's LPH lanes) that owns step k after reduce(), and the slot j it sits in
-  static __host__ __device__ constexpr int owner_sub(int k) { return LPH == 4 ? (k >> 1) : k * (LPH / 8); }
-  static __host__ __device__ constexpr int owner_slot(int k) { return LPH == 4 ? (k & 1) : 0; }
+  template <int NB> static __host__ __device__ constexpr int owner_sub(int k) { return NB > LPH ? k / kh<NB>() : k * (LPH / NB); }
+  template <int NB> static __host__ __device__ constexpr int owner_slot(int k) { return NB > LPH ? k % kh<NB>() : 0; }
 
   static __device__ __forceinline__ float sqrt_approx(float v) {
     float r; asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(v)); return r;
@@ -96,12 +99,12 @@ struct ScanCore {
   // independent parts of the arithmetic overlap; a missing step is an empty one and leaves the state as it is).
   // Returns the 0-based index within the batch of the step at which the criterion fired (c >= patience,
   // PAPER.md:157), or -1.
-  template <typename LoadML, typename LoadPV>
-  __device__ __forceinline__ int batch(int n, int lane, float tau, float phi, int patience, LoadML&& load_ml, LoadPV&& load_pv) {
+  template <int NB, typename LoadML, typename LoadPV>
+  __device__ __forceinline__ int batch_n(int n, int lane, float tau, float phi, int patience, LoadML&& load_ml, LoadPV&& load_pv) {
     // ---- the scalar chain: reference exponent and A_t, r_t = 2^(m_t - m) / A_t
-    float lt[kScanBatch], r[kScanBatch];
+    float lt[NB], r[NB];
 #pragma unroll
-    for (int k = 0; k < kScanBatch; ++k) {
+    for (int k = 0; k < NB; ++k) {
       float mt;
       load_ml(k, k < n, mt, lt[k]);                        // (-inf, 0) when the predicate is false
       const float mn = fmaxf(m_run, mt);
@@ -112,9 +115,9 @@ struct ScanCore {
       m_run = mn; l_run = l_new;
     }
     // ---- the recurrence x^(t) = x^(t-1) + r_t (P~V_t - l_t x^(t-1))   (l_t u^(t) = P~V_t)
-    float s[kScanBatch][3];
+    float s[NB][3];
 #pragma unroll
-    for (int k = 0; k < kScanBatch; ++k) {
+    for (int k = 0; k < NB; ++k) {
       float pv[CPL];
       load_pv(k, k < n, pv);                               // zeros when the predicate is false
       float sdd = 0.f, sad = 0.f, saa = 0.f;
@@ -126,23 +129,31 @@ struct ScanCore {
       }
       s[k][0] = sdd; s[k][1] = sad; s[k][2] = saa;
     }
-    reduce(s, lane);
+    reduce<NB>(s, lane);
+    constexpr int KH = kh<NB>();
     uint32_t votes[KH];
 #pragma unroll
     for (int j = 0; j < KH; ++j) votes[j] = __ballot_sync(0xffffffffu, stable_head(s[j], tau, phi));
     int fired = -1;
 #pragma unroll
-    for (int k = 0; k < kScanBatch; ++k) {
+    for (int k = 0; k < NB; ++k) {
       uint32_t need = 0;                                   // the lanes (one per head) that own step k
 #pragma unroll
-      for (int h = 0; h < G; ++h) need |= 1u << (h * LPH + owner_sub(k));
-      const bool stable = (votes[owner_slot(k)] & need) == need;     // AND over the group's heads (R2)
+      for (int h = 0; h < G; ++h) need |= 1u << (h * LPH + owner_sub<NB>(k));
+      const bool stable = (votes[owner_slot<NB>(k)] & need) == need;     // AND over the group's heads (R2)
       const int c_new = stable ? cnt + 1 : 0;              // Eq. 3
       const bool live = (k < n) && (fired < 0);
       cnt = live ? c_new : cnt;
       fired = (live && c_new >= patience) ? k : fired;
     }
     return fired;
+  }
+  // n <= kScanBatch steps: a half-size batch costs half, so short runs of arrived steps are decided sooner
+  template <typename LoadML, typename LoadPV>
+  __device__ __forceinline__ int batch(int n, int lane, float tau, float phi, int patience, LoadML&& load_ml, LoadPV&& load_pv) {
+    if (n <= kScanBatch / 4) return batch_n<kScanBatch / 4>(n, lane, tau, phi, patience, load_ml, load_pv);
+    if (n <= kScanBatch / 2) return batch_n<kScanBatch / 2>(n, lane, tau, phi, patience, load_ml, load_pv);
+    return batch_n<kScanBatch>(n, lane, tau, phi, patience, load_ml, load_pv);
   }
 };
 
