@@ -39,6 +39,7 @@ struct Params {
   float tau, phi;
   int32_t patience;
   int32_t stages, mbox_slots;
+  int32_t dyn;                                       // bf16 cluster kernel: steps claimed at run time instead of dealt round-robin
 #ifdef ART_TRACE
   uint8_t* trace;
 #endif

@@ -326,6 +326,9 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   p.scale_log2 = scale * 1.4426950408889634f;
   if (th) { p.tau = th->tau; p.phi = th->phi; p.patience = th->patience; }
   p.stages = pl.stages; p.mbox_slots = pl.mslots;
+  // With the detector on, the CTAs of a cluster are coupled through the mailbox window; claiming steps at run time
+  // keeps a CTA that shares its SM from holding the others back.  It pays for clusters of 2-4 (measured).
+  p.dyn = (tensor_core && mode != 0 && C >= 2 && C <= 4) ? 1 : 0;
 
   cudaError_t e;
   if (dynamic) {

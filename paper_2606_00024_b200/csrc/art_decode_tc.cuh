@@ -39,7 +39,7 @@ namespace art {
 namespace tc {
 
 #ifdef ART_TRACE
-#define TC_TRACE_INIT(tr, role) Tracer tr; tr.init(p.trace, 0, role, reinterpret_cast<volatile int*>(smem + sm.misc + 12))
+#define TC_TRACE_INIT(tr, role) Tracer tr; tr.init(p.trace, 0, role, reinterpret_cast<volatile int*>(smem + sm.misc + 20))
 #define TC_TRACE(tr, code, a, b) tr.ev(code, a, b)
 #else
 #define TC_TRACE_INIT(tr, role)
@@ -60,6 +60,8 @@ constexpr int kIterSlots = 16;               // softmax -> fold hand-over ring; 
 constexpr int kMaxStages = 6;
 // P^T (hi, lo) buffers: one per ring stage, except for G = 8 with the detector on, where shared memory only has room for two (block i
 // then uses buffer i & 1, free again once P~V_(i-2) is complete)
+// ring of the step numbers of the items in flight (>= stages + kPVSlots entries; 12 where every byte counts)
+__host__ __device__ constexpr int item_ring(int G, bool art32) { return (G == 8 && art32) ? 12 : 16; }
 __host__ __device__ constexpr int p_bufs(int G, int stages, bool art32) { return (G == 8 && art32) ? 2 : stages; }
 constexpr int kBoxBytes = 8192;              // one TMA box: 64 rows x 128 bytes
 constexpr int kFront = 12288;                // mapped bytes the S MMA may read below a K tile (3 x 32 rows)
@@ -79,7 +81,7 @@ struct IterSlot {            // what softmax hands to fold for one block
 };
 
 struct SmemMap {
-  uint32_t qb, pb, slots, sinfo, mbox, bars, misc, ring, total;
+  uint32_t qb, pb, slots, items, sinfo, mbox, bars, misc, ring, total;
   uint32_t full0, empty0, pfull0, sfull0, sfree0, pvfull0, pvfree0, done0, mbox0, nbars;
 };
 
@@ -91,6 +93,7 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   m.qb = off; off += kQBytes;
   m.pb = off; off += static_cast<uint32_t>(p_bufs(G, stages, art && PW == 32)) * 2u * p_buf_bytes(G);
   m.slots = off; off += kIterSlots * static_cast<uint32_t>(sizeof(IterSlot));
+  m.items = off; off += static_cast<uint32_t>(item_ring(G, art && PW == 32)) * 4u;
   m.sinfo = off; off += static_cast<uint32_t>(stages) * 8u;
   off = (off + 15u) & ~15u;                // mailbox rows are written with 16-byte st.async
   m.mbox = off; off += art ? static_cast<uint32_t>(mslots) * G * (2 + PW) * 4u : 0u;
@@ -104,14 +107,14 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   m.mbox0 = n; n += art ? mslots : 0;
   m.nbars = n;
   off += n * 8u;
-  m.misc = off; off += 16u;              // ctrl, loaded, tmem_ptr
+  m.misc = off; off += 24u;              // ctrl, loaded, tmem_ptr, next_step (leader), n_total
   off = (off + 1023u) & ~1023u;
   if (off < static_cast<uint32_t>(kFront)) off = kFront;
   m.ring = off; off += static_cast<uint32_t>(stages) * kStageBytes;
   m.total = off;
   return m;
 }
-constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8;
+constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8, kNext = 12, kNTotal = 16;
 
 // ----------------------------------------------------------------------------- tcgen05 / TMA wrappers
 
@@ -257,7 +260,11 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   const int L = p.seq_lens[b];
   const Trav tr = make_trav(p, b, g, L);
   const int Tn = tr.T;
-  const int n_c = (Tn > rank) ? (Tn - rank + C - 1) / C : 0;   // steps owned by this CTA
+  const int n_c = (Tn > rank) ? (Tn - rank + C - 1) / C : 0;   // steps of this CTA when they are dealt round-robin
+  const int n_lim = p.dyn ? 0x7fffffff : n_c;                 // items this CTA will process, if known up front
+  constexpr int kItemT = item_ring(G, MODE == 1);
+  int* item_t = reinterpret_cast<int*>(smem + sm.items);      // step number of item i (i mod kItemT)
+  const uint32_t a_ntotal = sbase + sm.misc + kNTotal;
 
 #ifdef ART_TRACE
   unsigned long long* cta_times = p.trace ? reinterpret_cast<unsigned long long*>(p.trace + 256 + static_cast<size_t>(kTraceCtas) * kTraceRoles * kTraceEvents * 16) + 4 * blockIdx.x : nullptr;
@@ -275,7 +282,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (rank == 0 && s < Tn) mbar_arrive_expect_tx(bar(sm.mbox0 + s), kSummaryBytes);   // armed for steps 1..M
       }
     }
-    st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_loaded, 0); st_volatile_s32(sbase + sm.misc + 12, 0);
+    st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_loaded, 0);
+    st_volatile_s32(sbase + sm.misc + kNext, 0); st_volatile_s32(a_ntotal, 0x7fffffff); st_volatile_s32(sbase + sm.misc + 20, 0);
     fence_mbar_init();
   }
   if (warp == kWarpMmaPV) tmem_alloc(a_tmem, kTmemCols);
@@ -303,11 +311,14 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     const int c = ld_ctrl_relaxed(a_ctrl);
     return c < 0 && t > -c;
   };
-  auto wait_or_stop = [&](uint32_t baddr, uint32_t parity, int t) -> bool {
-    while (!mbar_try_wait(baddr, parity)) { if (beyond_stop(t)) return false; }
+  // Every issued item runs through all roles (one beyond t* is dropped by the fold warps); a wait can only fail
+  // once the producer has issued its last item (known up front, n_lim, unless steps are claimed at run time
+  // or Algorithm 1 fires).
+  auto wait_item = [&](uint32_t baddr, uint32_t parity, int i) -> bool {
+    if constexpr (!ART) { mbar_wait(baddr, parity); return true; }          // detector off: every item arrives
+    while (!mbar_try_wait(baddr, parity)) { if (i >= ld_volatile_s32(a_ntotal)) return false; }
     return true;
   };
-  auto step_of = [&](int i) { return i * C + rank + 1; };
 
   // fold warps: this thread's output coordinate and the running (un-normalised) state; read by the epilogue
   const int fq = warp & 3;
@@ -321,47 +332,110 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     int it_issued = 0, loaded = 0, stage = 0;
     TC_TRACE_INIT(trc, 0);
     uint32_t ph = 0;                                          // (it / S) & 1
-    bool stop = false;
-    for (int i0 = 0; i0 < n_c && !stop; i0 += 32) {
-      const int i = i0 + lane;
-      unsigned long long mask = 0ull; int c1 = 0, c2 = 0;
-      if (i < n_c) {
-        const int blk = trav_block(tr, step_of(i));
-        mask = block_mask(p, L, blk);
-        if (mask) {
-          const int page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
-          if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = page * p.Hkv + g; }     // [page*Hkv + head][token][d]
-          else { c1 = g; c2 = page * kBlockTokens; }                             // [page*64 + token][head][d]
+    if (p.dyn) {
+      // ---- steps CLAIMED at run time from a counter in the leader's shared memory: a CTA that shares its SM takes
+      //      fewer steps than one that has an SM to itself, and nobody waits at the mailbox window for a slower CTA
+      int it = 0;
+      const uint32_t a_next = mapa(sbase + sm.misc + kNext, 0); // the cluster's claim counter lives in the leader
+      auto claim = [&]() -> int {                               // next unclaimed step, 1-based
+        uint32_t r;
+        asm volatile("atom.relaxed.cluster.shared::cluster.add.u32 %0, [%1], 1;" : "=r"(r) : "r"(a_next) : "memory");
+        return static_cast<int>(r) + 1;
+      };
+      // resolve a claimed step: validity, token mask, page (the table lookup is left in flight)
+      auto resolve = [&](int t, bool& valid, unsigned long long& mask, int& page) {
+        valid = t <= Tn && !beyond_stop(t);                     // exhausted, or beyond t* (A7: stop prefetching)
+        mask = 0ull; page = 0;
+        if (valid) {
+          const int blk = trav_block(tr, t);
+          mask = block_mask(p, L, blk);
+          if (mask) page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
         }
-      }
-      const int cnt = min(32, n_c - i0);
-      for (int kk = 0; kk < cnt; ++kk) {
-        const int it = i0 + kk, t = step_of(it);
-        const unsigned long long mask_k = __shfl_sync(0xffffffffu, mask, kk);
-        const int c1_k = __shfl_sync(0xffffffffu, c1, kk), c2_k = __shfl_sync(0xffffffffu, c2, kk);
-        if (it >= S && !wait_or_stop(bar(sm.empty0 + stage), ph ^ 1u, t)) stop = true;   // slot released?
-        if (!stop && beyond_stop(t)) stop = true;            // A7: stop issuing prefetch once fired
-        if (stop) break;
+      };
+      // claim -> page lookup -> TMA is software-pipelined: item A resolved, item B claimed, next claim issued
+      int tB = 0;
+      if (lane == 0) tB = claim();
+      int tA = __shfl_sync(0xffffffffu, tB, 0);
+      bool validA; unsigned long long maskA; int pageA;
+      resolve(tA, validA, maskA, pageA);
+      if (lane == 0) tB = claim();
+      while (validA) {
+        const int tN = __shfl_sync(0xffffffffu, tB, 0);
+        bool validB; unsigned long long maskB; int pageB;
+        resolve(tN, validB, maskB, pageB);
+        if (validB && lane == 0) tB = claim();
+        if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                  // slot released?
         if (lane == 0) {
-          TC_TRACE(trc, 1, group, t);
+          TC_TRACE(trc, 1, group, tA);
           const uint32_t fb = bar(sm.full0 + stage);
           const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
-          sinfo[stage] = mask_k;
-          if (mask_k == 0ull) {
-            mbar_arrive(fb);                                 // nothing to load: an all-masked step
+          item_t[it % kItemT] = tA;
+          sinfo[stage] = maskA;
+          if (maskA == 0ull) {
+            mbar_arrive(fb);                                   // nothing to load: an all-masked step
           } else {
+            int c1, c2;
+            if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = pageA * p.Hkv + g; }   // [page*Hkv + head][token][d]
+            else { c1 = g; c2 = pageA * kBlockTokens; }                           // [page*64 + token][head][d]
             mbar_arrive_expect_tx(fb, kStageBytes);
-            tma_load_box(dst, &tmK, 0, c1_k, c2_k, fb);
-            tma_load_box(dst + kBoxBytes, &tmK, 64, c1_k, c2_k, fb);
-            tma_load_box(dst + 2 * kBoxBytes, &tmV, 0, c1_k, c2_k, fb);
-            tma_load_box(dst + 3 * kBoxBytes, &tmV, 64, c1_k, c2_k, fb);
+            tma_load_box(dst, &tmK, 0, c1, c2, fb);
+            tma_load_box(dst + kBoxBytes, &tmK, 64, c1, c2, fb);
+            tma_load_box(dst + 2 * kBoxBytes, &tmV, 0, c1, c2, fb);
+            tma_load_box(dst + 3 * kBoxBytes, &tmV, 64, c1, c2, fb);
           }
         }
-        if (mask_k != 0ull) ++loaded;
-        it_issued = it + 1;
+        if (maskA != 0ull) ++loaded;
+        ++it;
         if (++stage == S) { stage = 0; ph ^= 1u; }
+        tA = tN; validA = validB; maskA = maskB; pageA = pageB;
+      }
+      it_issued = it;
+    } else {
+      // ---- steps dealt round-robin: CTA c owns steps c+1, c+1+C, ...; 32 of them are resolved at a time
+      auto step_of = [&](int i) { return i * C + rank + 1; };
+      bool stop = false;
+      for (int i0 = 0; i0 < n_c && !stop; i0 += 32) {
+        const int i = i0 + lane;
+        unsigned long long mask = 0ull; int c1 = 0, c2 = 0;
+        if (i < n_c) {
+          const int blk = trav_block(tr, step_of(i));
+          mask = block_mask(p, L, blk);
+          if (mask) {
+            const int page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
+            if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = page * p.Hkv + g; }     // [page*Hkv + head][token][d]
+            else { c1 = g; c2 = page * kBlockTokens; }                             // [page*64 + token][head][d]
+          }
+        }
+        const int cnt = min(32, n_c - i0);
+        for (int kk = 0; kk < cnt; ++kk) {
+          const int it = i0 + kk, t = step_of(it);
+          const unsigned long long mask_k = __shfl_sync(0xffffffffu, mask, kk);
+          const int c1_k = __shfl_sync(0xffffffffu, c1, kk), c2_k = __shfl_sync(0xffffffffu, c2, kk);
+          if (beyond_stop(t)) { stop = true; break; }          // A7: stop issuing prefetch once fired
+          if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                // slot released?
+          if (lane == 0) {
+            TC_TRACE(trc, 1, group, t);
+            const uint32_t fb = bar(sm.full0 + stage);
+            const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
+            item_t[it % kItemT] = t;
+            sinfo[stage] = mask_k;
+            if (mask_k == 0ull) {
+              mbar_arrive(fb);                                 // nothing to load: an all-masked step
+            } else {
+              mbar_arrive_expect_tx(fb, kStageBytes);
+              tma_load_box(dst, &tmK, 0, c1_k, c2_k, fb);
+              tma_load_box(dst + kBoxBytes, &tmK, 64, c1_k, c2_k, fb);
+              tma_load_box(dst + 2 * kBoxBytes, &tmV, 0, c1_k, c2_k, fb);
+              tma_load_box(dst + 3 * kBoxBytes, &tmV, 64, c1_k, c2_k, fb);
+            }
+          }
+          if (mask_k != 0ull) ++loaded;
+          it_issued = it + 1;
+          if (++stage == S) { stage = 0; ph ^= 1u; }
+        }
       }
     }
+    if (lane == 0) st_volatile_s32(a_ntotal, it_issued);
     if (lane == 0) st_volatile_s32(a_loaded, loaded);
 #ifdef ART_TRACE
     if (lane == 0 && cta_times) cta_times[2] = trace_now();
@@ -375,10 +449,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       const uint64_t dQ = kDescNoSw | desc_strides(kQLbo, kQSbo);
       const uint32_t qb = sbase + sm.qb;
       int st = 0; uint32_t ph = 0;
-      for (int i = 0; i < n_c; ++i) {
-        const int q = i & (NS - 1), t = step_of(i);
-        if (!wait_or_stop(bar(sm.full0 + st), ph, t)) break;
-        if (i >= NS && !wait_or_stop(bar(sm.sfree0 + q), ((i / NS) - 1) & 1, t)) break;
+      for (int i = 0; i < n_lim; ++i) {
+        const int q = i & (NS - 1);
+        if (!wait_item(bar(sm.full0 + st), ph, i)) break;
+        if (i >= NS && !wait_item(bar(sm.sfree0 + q), ((i / NS) - 1) & 1, i)) break;
         tc_fence_after();
         // M = 128 rows are read starting 32 q token rows BELOW the tile (tokens 0-31 -> TMEM lanes 32q..32q+31,
         // columns +0) and once more 32 rows further up (tokens 32-63 -> the same lanes, columns +16).  The
@@ -404,10 +478,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       const uint64_t dV = kDescSw128 | desc_strides(kBoxBytes, 1024);  // V tile as V^T: MN-major, 128-B swizzle
       const uint64_t dP = kDescNoSw | desc_strides(LBO_P, 128);
       int st = 0; uint32_t ph = 0;
-      for (int i = 0; i < n_c; ++i) {
-        const int ps = i & (NP - 1), t = step_of(i);
-        if (!wait_or_stop(bar(sm.pfull0 + st), ph, t)) break;
-        if (i >= NP && !wait_or_stop(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1, t)) break;
+      for (int i = 0; i < n_lim; ++i) {
+        const int ps = i & (NP - 1);
+        if (!wait_item(bar(sm.pfull0 + st), ph, i)) break;
+        if (i >= NP && !wait_item(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1, i)) break;
         tc_fence_after();
         const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
         const uint32_t pb = sbase + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF;
@@ -429,9 +503,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     const int q = warp - kWarpSoftmax0;                       // TMEM lane quadrant == warp % 4; owns blocks i = q (mod 4)
     const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
     int st = q % S;                                           // ring stage of block i
-    for (int i = q; i < n_c; i += NS) {
-      const int t = step_of(i);
-      if (!wait_or_stop(bar(sm.sfull0 + q), (i / NS) & 1, t)) break;
+    for (int i = q; i < n_lim; i += NS) {
+      if (!wait_item(bar(sm.sfull0 + q), (i / NS) & 1, i)) break;
       tc_fence_after();
       float s0[G], s1[G];
       tmem_ld<G>(taddr, s0);
@@ -441,7 +514,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
       // P^T buffer i & 1 is read by the P.V MMA of block i - 2: wait until that one is complete
-      if (kTwoPBufs && i >= 2 && !wait_or_stop(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1, t)) break;
+      if (kTwoPBufs && i >= 2 && !wait_item(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1, i)) break;
       const unsigned long long vmask = sinfo[st];             // written before the loads the S MMA waited for
       const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
       float mb[G];
@@ -495,6 +568,11 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     // ===================================================== A5 / A6: publish step summaries, merge P~V_t
     const uint32_t tlane = static_cast<uint32_t>(fq * 32) << 16;
     TC_TRACE_INIT(trf, 1);
+    auto release_pv = [&](int i) {                           // the tensor-memory slot of item i is free again
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(sm.pvfree0 + (i & (NP - 1))));
+    };
     // merge block i (its P~V_t is relative to its own block maximum) into the running state
     auto fold = [&](int i) {
       tc_fence_after();
@@ -513,31 +591,36 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
           m_tot[h] = mn;
         }
       }
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.pvfree0 + (i & (NP - 1))));
-      if (tid == 0) TC_TRACE(trf, 5, i, step_of(i));
+      release_pv(i);
+      if (tid == 0) TC_TRACE(trf, 5, i, item_t[i % kItemT]);
     };
     if constexpr (!ART) {
-      for (int i = 0; i < n_c; ++i) {
-        mbar_wait(bar(sm.pvfull0 + (i & (NP - 1))), (i / NP) & 1);
+      for (int i = 0; i < n_lim; ++i) {
+        if (!wait_item(bar(sm.pvfull0 + (i & (NP - 1))), (i / NP) & 1, i)) break;
         fold(i);
       }
     } else {
       int pub = 0, fld = 0;
       bool pub_ready = false;                                 // P~V of block `pub` is complete in tensor memory
-      while (fld < n_c) {
+      while (fld < n_lim) {
+        const int ntot = ld_volatile_s32(a_ntotal);
+        if (fld >= ntot) break;
         const int c = ld_ctrl_relaxed(a_ctrl);
-        if (c < 0 && step_of(fld) > -c) break;                // everything from here on lies beyond t*
-        // ---- merge the oldest unfolded block once the decision for the steps before it is known
-        if (fld < pub && (c < 0 || c >= step_of(fld) - 1)) { fold(fld); ++fld; continue; }
+        // ---- merge the oldest unfolded block once the decision for the steps before it is known; one that
+        //      lies beyond t* is dropped (its tensor-memory slot is released, nothing is merged)
+        if (fld < pub) {
+          const int tf = item_t[fld % kItemT];
+          if (c < 0 && tf > -c) { release_pv(fld); ++fld; continue; }
+          if (c < 0 || c >= tf - 1) { fold(fld); ++fld; continue; }
+        }
         // ---- publish the summary of the next finished block (never waits for a decision on itself)
-        if (pub < n_c && pub - fld < NP) {
+        if (pub < ntot && pub < n_lim && pub - fld < NP) {
           const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
           const uint32_t par = (pub / NP) & 1;
           if (!pub_ready) pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
-          const int t = step_of(pub);
-          if (pub_ready && c >= 0 && c >= t - M) {            // mailbox slot free: step t - M has been scanned
+          if (pub_ready && c < 0) { ++pub; pub_ready = false; continue; }   // fired: an unpublished step lies beyond t*
+          const int t = pub_ready ? item_t[pub % kItemT] : 0;
+          if (pub_ready && c >= t - M) {                      // mailbox slot free: step t - M has been scanned
             const int slot_i = (t - 1) & (M - 1);
             tc_fence_after();
             float pv[G];

@@ -145,7 +145,8 @@ def test_patience_inf_equals_off():
     o1, s1, _ = a.run_workload(wc, art=True, patience=a.ART_PATIENCE_INF, split=2)
     o0, s0, _ = a.run_workload(wc, art=False, split=2)
     assert torch.equal(s1, s0)
-    assert torch.equal(o1, o0)                  # same fold order => bit-identical
+    # with the detector on, clusters of 2-4 claim steps at run time: the merge order, hence the last bits, differ
+    assert (o1 - o0).abs().max() <= 1e-5 * o0.abs().max()
 
 
 def test_ablation_switches_and_extremes():
@@ -171,7 +172,11 @@ def test_split_invariance_and_determinism():
         assert torch.equal(s, ref_s)
         assert (o - ref_o).abs().max() <= 1e-5 * ref_o.abs().max()
         o2, s2, _ = a.run_workload(wc, tau=1e-3, split=split)
-        assert torch.equal(o, o2) and torch.equal(s, s2)
+        assert torch.equal(s, s2)                   # stop blocks are bit-deterministic for every schedule
+        if split in (1, 8, 16):                     # static dealing: bit-identical outputs as well
+            assert torch.equal(o, o2)
+        else:                                       # steps claimed at run time: the merge order may differ
+            assert (o - o2).abs().max() <= 1e-5 * o.abs().max()
 
 
 def test_edge_cases():
