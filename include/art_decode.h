@@ -145,7 +145,9 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
                               int32_t* stop_block_host, void* workspace, size_t workspace_bytes,
                               void* cuda_stream);
 
-/* DEVICE scratch bytes art_decode_attention_host needs for this problem (0 on a bad desc). */
+/* DEVICE scratch bytes that cover every entry point for this problem: the staging area of
+ * art_decode_attention_host plus the control blocks, mailboxes and partial states of the dynamically
+ * scheduled kernel (split == ART_SPLIT_DYNAMIC).  0 on a bad desc.  Needs no CUDA device. */
 size_t art_workspace_bytes(const art_desc_t* desc);
 
 /* Cluster size the library would pick for desc->split == 0 (needs a CUDA device); <0 = error code. */

@@ -219,6 +219,19 @@ def test_error_codes_on_device():
     assert a.art_query_split(a.make_desc(w, split=-1), True) == 0   # dynamic scheduler: no fixed cluster
 
 
+def test_dynamic_scheduler_needs_workspace():
+    a = art()
+    w = small(1).to("cuda")
+    desc = a.make_desc(w, split=a.ART_SPLIT_DYNAMIC)
+    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), device="cuda")
+    stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device="cuda")
+    tiny = torch.empty(256, dtype=torch.uint8, device="cuda")
+    with pytest.raises(a.ArtError) as e:
+        a.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table, None, w.seq_lens, out, stop, workspace=tiny)
+    assert e.value.status == -5                 # ART_ERR_WORKSPACE: too small, nothing launched
+    assert a.art_workspace_bytes(desc) > 256
+
+
 def test_host_entry_point():
     """art_decode_attention_host: pinned host inputs/outputs, KV caches on the device."""
     a = art()
