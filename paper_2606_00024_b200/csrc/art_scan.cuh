@@ -99,14 +99,14 @@ struct ScanCore {
   // independent parts of the arithmetic overlap; a missing step is an empty one and leaves the state as it is).
   // Returns the 0-based index within the batch of the step at which the criterion fired (c >= patience,
   // PAPER.md:157), or -1.
-  template <int NB, typename LoadML, typename LoadPV>
+  template <int NB, bool FULL, typename LoadML, typename LoadPV>      // FULL: n == NB, nothing is predicated
   __device__ __forceinline__ int batch_n(int n, int lane, float tau, float phi, int patience, LoadML&& load_ml, LoadPV&& load_pv) {
     // ---- the scalar chain: reference exponent and A_t, r_t = 2^(m_t - m) / A_t
     float lt[NB], r[NB];
 #pragma unroll
     for (int k = 0; k < NB; ++k) {
       float mt;
-      load_ml(k, k < n, mt, lt[k]);                        // (-inf, 0) when the predicate is false
+      load_ml(k, FULL || k < n, mt, lt[k]);                // (-inf, 0) when the predicate is false
       const float mn = fmaxf(m_run, mt);
       const float al = (m_run == mn) ? 1.f : fast_exp2(m_run - mn);
       const float be = (mt == kNegInf) ? 0.f : fast_exp2(mt - mn);   // a step with no valid token changes nothing (R8)
@@ -119,7 +119,7 @@ struct ScanCore {
 #pragma unroll
     for (int k = 0; k < NB; ++k) {
       float pv[CPL];
-      load_pv(k, k < n, pv);                               // zeros when the predicate is false
+      load_pv(k, FULL || k < n, pv);                       // zeros when the predicate is false
       float sdd = 0.f, sad = 0.f, saa = 0.f;
 #pragma unroll
       for (int j = 0; j < CPL; ++j) {
@@ -134,6 +134,16 @@ struct ScanCore {
     uint32_t votes[KH];
 #pragma unroll
     for (int j = 0; j < KH; ++j) votes[j] = __ballot_sync(0xffffffffu, stable_head(s[j], tau, phi));
+    // far from convergence no step of the batch is stable: the counter is simply back at 0 (Eq. 3)
+    bool any = false;
+#pragma unroll
+    for (int k = 0; k < NB; ++k) {
+      uint32_t need = 0;
+#pragma unroll
+      for (int h = 0; h < G; ++h) need |= 1u << (h * LPH + owner_sub<NB>(k));
+      any |= (FULL || k < n) && (votes[owner_slot<NB>(k)] & need) == need;
+    }
+    if (!any) { cnt = (n > 0) ? 0 : cnt; return -1; }
     int fired = -1;
 #pragma unroll
     for (int k = 0; k < NB; ++k) {
@@ -142,7 +152,7 @@ struct ScanCore {
       for (int h = 0; h < G; ++h) need |= 1u << (h * LPH + owner_sub<NB>(k));
       const bool stable = (votes[owner_slot<NB>(k)] & need) == need;     // AND over the group's heads (R2)
       const int c_new = stable ? cnt + 1 : 0;              // Eq. 3
-      const bool live = (k < n) && (fired < 0);
+      const bool live = (FULL || k < n) && (fired < 0);
       cnt = live ? c_new : cnt;
       fired = (live && c_new >= patience) ? k : fired;
     }
@@ -151,9 +161,10 @@ struct ScanCore {
   // n <= kScanBatch steps: a half-size batch costs half, so short runs of arrived steps are decided sooner
   template <typename LoadML, typename LoadPV>
   __device__ __forceinline__ int batch(int n, int lane, float tau, float phi, int patience, LoadML&& load_ml, LoadPV&& load_pv) {
-    if (n <= kScanBatch / 4) return batch_n<kScanBatch / 4>(n, lane, tau, phi, patience, load_ml, load_pv);
-    if (n <= kScanBatch / 2) return batch_n<kScanBatch / 2>(n, lane, tau, phi, patience, load_ml, load_pv);
-    return batch_n<kScanBatch>(n, lane, tau, phi, patience, load_ml, load_pv);
+    if (n <= kScanBatch / 4) return batch_n<kScanBatch / 4, false>(n, lane, tau, phi, patience, load_ml, load_pv);
+    if (n <= kScanBatch / 2) return batch_n<kScanBatch / 2, false>(n, lane, tau, phi, patience, load_ml, load_pv);
+    if (n == kScanBatch) return batch_n<kScanBatch, true>(n, lane, tau, phi, patience, load_ml, load_pv);
+    return batch_n<kScanBatch, false>(n, lane, tau, phi, patience, load_ml, load_pv);
   }
 };
 
