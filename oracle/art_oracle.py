@@ -338,3 +338,52 @@ def art_decode_attention_oracle(q, k_cache, v_cache, block_table, seq_lens, *,
         stop[b, g] = r.stop_block
         results[(b, g)] = r
     return out, stop, results
+
+
+# --------------------------------------------------------------------------- base-policy block list
+
+def block_scores_oracle(q, k_cache, block_table, seq_lens, *, num_kv_heads: int,
+                        layout: int = LAYOUT_HND) -> np.ndarray:
+    """Block priority of the scored base policy the paper orders importance-first: for every
+    (sequence b, KV head g, logical block) the MEAN over the group's G query heads and the block's valid
+    tokens (j < L) of q_h . k_j, in fp64.  (The paper's SnapKV scores need prefill attention maps, which do
+    not exist here; this stand-in is BASELINE.json's "mean q.k score".)
+
+    Plain loops over blocks, one dot product per (head, token): the definition written out.
+    Returns [B, Hkv, max_blocks] float64; blocks at or beyond ceil(L / 64) get -inf.
+    """
+    q = np.asarray(q, dtype=np.float64)
+    B, Hq, d = q.shape
+    Hkv = int(num_kv_heads)
+    G = Hq // Hkv
+    max_blocks = int(np.asarray(block_table).shape[1])
+    scores = np.full((B, Hkv, max_blocks), -np.inf)
+    for b in range(B):
+        L = int(seq_lens[b])
+        nb = -(-L // BLOCK_TOKENS) if L > 0 else 0
+        for g in range(Hkv):
+            for blk in range(nb):
+                tile = gather_group_blocks(k_cache, layout, block_table[b], g, [blk])[0]      # [64, d]
+                n_valid = min(BLOCK_TOKENS, L - blk * BLOCK_TOKENS)
+                total = 0.0
+                for h in range(g * G, (g + 1) * G):
+                    total += float((tile[:n_valid] @ q[b, h]).sum())
+                scores[b, g, blk] = total / (G * n_valid)
+    return scores
+
+
+def topk_blocks_oracle(scores: np.ndarray, seq_lens, top_k: int):
+    """Importance-first list (reading R10): the top_k candidate blocks by DESCENDING score,
+    ties -> lower block index first.  Returns (lists [B, Hkv, top_k] int64 padded with -1, counts [B, Hkv])."""
+    B, Hkv, _ = scores.shape
+    lists = np.full((B, Hkv, max(int(top_k), 0)), -1, dtype=np.int64)
+    counts = np.zeros((B, Hkv), dtype=np.int64)
+    for b in range(B):
+        L = int(seq_lens[b])
+        nb = -(-L // BLOCK_TOKENS) if L > 0 else 0
+        for g in range(Hkv):
+            cand = sorted(range(nb), key=lambda blk: (-scores[b, g, blk], blk))
+            k = min(int(top_k), nb)
+            lists[b, g, :k] = cand[:k]
+            counts[b, g] = k
+    return lists, counts
