@@ -145,6 +145,23 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
                               int32_t* stop_block_host, void* workspace, size_t workspace_bytes,
                               void* cuda_stream);
 
+/*
+ * Base-policy side (scored methods are walked importance-first through "an auxiliary index
+ * mapping for indirect addressing"): builds that mapping on the device.
+ *   block_scores[b, g, blk] = mean over the G query heads of the group and over the valid tokens (j < L) of block
+ *                             blk of q_h . k_j (fp32); -inf for blocks at or beyond ceil(L / 64)
+ *   eligible_blocks[b, g, :] = the min(top_k, ceil(L / 64)) blocks with the largest score, in DESCENDING score,
+ *                             ties -> lower block index first (reading R10); eligible_counts[b, g] = their number
+ * The outputs are what art_decode_attention takes with policy == LIST.  Uses desc->{batch, num_q_heads,
+ * num_kv_heads, head_dim, block_tokens, dtype, kv_layout, max_blocks_per_seq (<= 4096), max_eligible (row stride
+ * of eligible_blocks, >= top_k)}.  q, k_cache, block_table, seq_lens as above; block_scores DEVICE float32
+ * [B, Hkv, max_blocks_per_seq]; eligible_blocks DEVICE int32 [B, Hkv, max_eligible]; eligible_counts DEVICE
+ * int32 [B, Hkv].  Enqueues two kernels on cuda_stream and returns.  Entries beyond the count are not written.
+ */
+int art_topk_blocks(const art_desc_t* desc, const void* q, const void* k_cache, const int32_t* block_table,
+                    const int32_t* seq_lens, int32_t top_k, float* block_scores, int32_t* eligible_blocks,
+                    int32_t* eligible_counts, void* cuda_stream);
+
 /* DEVICE scratch bytes that cover every entry point for this problem: the staging area of
  * art_decode_attention_host plus the control blocks, mailboxes and partial states of the dynamically
  * scheduled kernel (split == ART_SPLIT_DYNAMIC).  0 on a bad desc.  Needs no CUDA device. */

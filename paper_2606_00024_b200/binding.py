@@ -71,6 +71,8 @@ def load_library():
     lib.art_decode_attention_host.restype = C.c_int
     lib.art_decode_attention_host.argtypes = [C.POINTER(ArtDesc), vp, vp, vp, i32p, i32p, i32p,
                                               C.POINTER(ArtThresholds), f32p, i32p, vp, C.c_size_t, vp]
+    lib.art_topk_blocks.restype = C.c_int
+    lib.art_topk_blocks.argtypes = [C.POINTER(ArtDesc), vp, vp, i32p, i32p, C.c_int32, f32p, i32p, i32p, vp]
     lib.art_workspace_bytes.restype = C.c_size_t
     lib.art_workspace_bytes.argtypes = [C.POINTER(ArtDesc)]
     lib.art_query_split.restype = C.c_int
@@ -161,6 +163,16 @@ def art_decode_attention_host(desc, q_host, k_cache, v_cache, block_table_host, 
         _ptr(workspace), workspace.numel() * workspace.element_size(), _stream_ptr(stream))
     if rc != 0:
         raise ArtError(rc, "art_decode_attention_host")
+
+
+def art_topk_blocks(desc, q, k_cache, block_table, seq_lens, top_k, block_scores, eligible_blocks, eligible_counts,
+                    stream=None) -> None:
+    """Importance-first block list of the scored base policy, built on the device (include/art_decode.h)."""
+    rc = load_library().art_topk_blocks(C.byref(desc), _ptr(q), _ptr(k_cache), _ptr(block_table), _ptr(seq_lens),
+                                        int(top_k), _ptr(block_scores), _ptr(eligible_blocks), _ptr(eligible_counts),
+                                        _stream_ptr(stream))
+    if rc != 0:
+        raise ArtError(rc, "art_topk_blocks")
 
 
 # ------------------------------------------------------------------ convenience (argument marshalling only)

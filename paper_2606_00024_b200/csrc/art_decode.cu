@@ -12,6 +12,7 @@
 #include "art_decode_simt.cuh"
 #include "art_decode_tc.cuh"
 #include "art_decode_ws_kernel.cuh"
+#include "art_policy.cuh"
 
 namespace art {
 
@@ -459,6 +460,55 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
   ok &= cudaMemcpyAsync(stop_block_host, ws + h.stop, B * Hkv * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   ok &= cudaStreamSynchronize(st) == cudaSuccess;
   if (!ok) { cudaGetLastError(); return ART_ERR_CUDA; }
+  return ART_OK;
+}
+
+// ----------------------------------------------------------------------------- base-policy list (A1's input)
+
+int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, const int32_t* block_table,
+                    const int32_t* seq_lens, int32_t top_k, float* block_scores, int32_t* eligible_blocks,
+                    int32_t* eligible_counts, void* cuda_stream) {
+  if (!d || !q || !k_cache || !block_table || !seq_lens || !block_scores || !eligible_blocks || !eligible_counts) return ART_ERR_NULL;
+  if (d->batch < 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads) return ART_ERR_SHAPE;
+  const int G = d->num_q_heads / d->num_kv_heads;
+  if (G != 1 && G != 2 && G != 4 && G != 8) return ART_ERR_SHAPE;
+  if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
+  if (!((d->dtype == ART_DTYPE_F32 && d->head_dim == 64) || (d->dtype == ART_DTYPE_BF16 && d->head_dim == 128))) return ART_ERR_DTYPE;
+  if (d->kv_layout != ART_LAYOUT_HND && d->kv_layout != ART_LAYOUT_NHD) return ART_ERR_SHAPE;
+  if (top_k < 0 || top_k > d->max_eligible) return ART_ERR_SHAPE;
+  if (d->max_blocks_per_seq <= 0 || d->max_blocks_per_seq > art::policy::kMaxSortBlocks) return ART_ERR_SHAPE;
+  if ((reinterpret_cast<uintptr_t>(q) & 15u) || (reinterpret_cast<uintptr_t>(k_cache) & 15u)) return ART_ERR_ALIGN;
+  int rc = art::check_arch();
+  if (rc != ART_OK) return rc;
+  const int groups = d->batch * d->num_kv_heads;
+  if (groups == 0) return ART_OK;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+
+  art::policy::ScoreParams sp = {};
+  sp.q = q; sp.k = static_cast<const uint8_t*>(k_cache); sp.block_table = block_table; sp.seq_lens = seq_lens;
+  sp.scores = block_scores; sp.batch = d->batch; sp.Hq = d->num_q_heads; sp.Hkv = d->num_kv_heads;
+  sp.max_blocks = d->max_blocks_per_seq; sp.layout = d->kv_layout;
+  const int64_t row = art::kRowBytes;
+  if (d->kv_layout == ART_LAYOUT_HND) { sp.token_stride = row; sp.head_stride = row * art::kBlockTokens; sp.page_stride = sp.head_stride * d->num_kv_heads; }
+  else { sp.head_stride = row; sp.token_stride = row * d->num_kv_heads; sp.page_stride = sp.token_stride * art::kBlockTokens; }
+  const dim3 grid(static_cast<unsigned>(groups), static_cast<unsigned>((d->max_blocks_per_seq + art::policy::kScoreWarps - 1) / art::policy::kScoreWarps));
+  const dim3 block(art::policy::kScoreWarps * 32);
+#define ART_SCORE_CASE(GG)                                                                                          \
+  if (G == GG) {                                                                                                    \
+    if (d->dtype == ART_DTYPE_BF16) art::policy::art_block_scores_kernel<__nv_bfloat16, 128, GG><<<grid, block, 0, st>>>(sp); \
+    else art::policy::art_block_scores_kernel<float, 64, GG><<<grid, block, 0, st>>>(sp);                            \
+  }
+  ART_SCORE_CASE(1) ART_SCORE_CASE(2) ART_SCORE_CASE(4) ART_SCORE_CASE(8)
+#undef ART_SCORE_CASE
+  if (cudaGetLastError() != cudaSuccess) return ART_ERR_CUDA;
+
+  art::policy::TopkParams tp = {};
+  tp.scores = block_scores; tp.seq_lens = seq_lens; tp.lists = eligible_blocks; tp.counts = eligible_counts;
+  tp.Hkv = d->num_kv_heads; tp.max_blocks = d->max_blocks_per_seq; tp.max_elig = d->max_eligible; tp.top_k = top_k;
+  int n = 1;
+  while (n < d->max_blocks_per_seq) n <<= 1;
+  art::policy::art_topk_kernel<<<groups, 256, static_cast<size_t>(n) * 8, st>>>(tp);
+  if (cudaGetLastError() != cudaSuccess) return ART_ERR_CUDA;
   return ART_OK;
 }
 
