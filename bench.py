@@ -336,6 +336,35 @@ def run_study(args):
         torch.cuda.empty_cache()
 
 
+def run_policy(args):
+    """the scored base policy's block list built on the device (art_topk_blocks) on configs[2]
+    and configs[3b]: time, K bytes streamed (every K row once: groups x blocks x 16 KiB) against the HBM peak."""
+    import torch
+    from workloads import generators as gen
+    import paper_2606_00024_b200 as art
+    peak, which = peaks()
+    for index, sub in ((2, "a"), (3, "b")):
+        w = gen.config(index, sub=sub, device="cuda")
+        torch.cuda.synchronize()
+        maxb = int(w.block_table.shape[1]); k = int(w.eligible_blocks.shape[2])
+        scores = torch.empty((w.batch, w.num_kv_heads, maxb), dtype=torch.float32, device="cuda")
+        lists = torch.empty((w.batch, w.num_kv_heads, k), dtype=torch.int32, device="cuda")
+        counts = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device="cuda")
+        desc = art.make_desc(w)
+        fn = lambda: art.art_topk_blocks(desc, w.q, w.k_cache, w.block_table, w.seq_lens, k, scores, lists, counts)
+        ms = time_loop(fn, args.steps, args.warmup)
+        us = ms * 1e3 / args.steps
+        nblocks = int(((w.seq_lens.to(torch.int64) + 63) // 64).sum()) * w.num_kv_heads
+        kbytes = nblocks * 16384
+        agree = float((lists == w.eligible_blocks).float().mean())
+        print(json.dumps({"policy": "art_topk_blocks", "workload": w.name, "groups": w.batch * w.num_kv_heads, "top_k": k,
+                          "us": round(us, 1), "k_bytes": kbytes, "gbs": round(kbytes / (us * 1e-6) / 1e9, 1),
+                          "frac_of_peak": round(kbytes / (us * 1e-6) / 1e9 / peak, 4), "peak_gbs": peak, "peak_kind": which,
+                          "agrees_with_host_recipe": round(agree, 4)}), flush=True)
+        del w
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -343,6 +372,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="art", choices=["art", "reference"])
     ap.add_argument("--report", action="store_true")
+    ap.add_argument("--policy", action="store_true", help="time art_topk_blocks (SURVEY 8(f).3)")
     ap.add_argument("--study", action="store_true", help="probe-vs-full, ablation and sensitivity sweeps (SURVEY 8(f))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
@@ -362,6 +392,9 @@ def main():
         return
     if args.study:
         run_study(args)
+        return
+    if args.policy:
+        run_policy(args)
         return
 
     import torch

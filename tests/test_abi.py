@@ -26,7 +26,7 @@ def declared_symbols():
 def test_every_declared_symbol_is_exported(art):
     lib = art.load_library()
     syms = declared_symbols()
-    assert {"art_decode_attention", "art_decode_attention_off", "art_decode_attention_host",
+    assert {"art_decode_attention", "art_decode_attention_off", "art_decode_attention_host", "art_topk_blocks",
             "art_workspace_bytes", "art_query_split", "art_status_string", "art_version"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
