@@ -15,6 +15,7 @@
 // bounded number of prefetched-then-discarded blocks, which are counted in blocks_loaded.
 #pragma once
 #include "art_common.cuh"
+#include "art_scan.cuh"
 
 namespace art {
 namespace simt {
@@ -417,69 +418,57 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
     };
 
     if (rank == 0) {
-      // ---- leader: Algorithm 1's loop over steps, on summaries
-      float m_run = kNegInf, l_run = 0.f, x[CPL];
+      // ---- leader: Algorithm 1's loop over steps, on summaries, in batches (art_scan.cuh).
+      // The leader's own steps do not arrive by themselves: the scan warp moves each of them from the summary
+      // buffers into its mailbox slot first, then every step of the group is read from the mailbox alike.
+      using Scan = ScanCore<G, PW>;
+      Scan sc; sc.init();
+      int t = 1, t_stop = 0, own_next = 0;                   // own_next: next local iteration to move (step own_next * C + 1)
+      while (t <= Tn) {
+        while (own_next < n_c) {
+          const int ts = own_next * C + 1;
+          if (ts > t - 1 + M) break;                         // its slot still holds step ts - M, not scanned yet
+          if (ts != t && !mbar_test_wait(bar(sm.sumready0 + (own_next & 1)), (own_next >> 1) & 1)) break;   // not finished: later
+          float mt, lt, pv[CPL];
+          merge_local(own_next, ts, mt, lt, pv);             // waits if the scan cannot go on without it (ts == t)
+          float* mb = mbox + static_cast<size_t>((ts - 1) % M) * G * ROWF + h * ROWF;
+          if (sub == 0) { mb[0] = mt; mb[1] = lt; }
 #pragma unroll
-      for (int j = 0; j < CPL; ++j) x[j] = 0.f;              // x^(0) = 0 (Alg. 1 l.1)
-      int cnt = 0, t_stop = 0;                               // c^(0) = 0 (l.2)
-      uint32_t phasebits = 0;
-      for (int t = 1; t <= Tn; ++t) {
-        const int owner = (t - 1) % C;
-        float mt, lt, pv[CPL];
-        if (owner == 0) {
-          merge_local((t - 1) / C, t, mt, lt, pv);
-        } else {
-          const int slot = (t - 1) % M;
-          while (!mbar_try_wait_cluster(bar(sm.mbox0 + slot), (phasebits >> slot) & 1u)) {}
-          phasebits ^= 1u << slot;
-          const float* mb = mbox + static_cast<size_t>(slot) * G * ROWF + h * ROWF;
-          mt = mb[0]; lt = mb[1];
-#pragma unroll
-          for (int j = 0; j < CPL; ++j) pv[j] = mb[2 + sub + LPH * j];
+          for (int j = 0; j < CPL; ++j) mb[2 + sub + LPH * j] = pv[j];
+          mbar_arrive(bar(sm.mbox0 + (ts - 1) % M));         // 32 arrivals complete the slot, as for a remote step
+          ++own_next;
         }
-        // streaming update in recurrence form: x^(t) - x^(t-1) = (l_t / A_t) P(u^(t) - o^(t-1))
-        // (PAPER.md:320, :361), with l_t u^(t) = P~V_t and everything relative to the running max.
-        float sdd = 0.f, sad = 0.f, saa = 0.f, sbb = 0.f;
-        if (mt != kNegInf) {                                 // a step with no valid token changes nothing (R8)
-          const float mn = fmaxf(m_run, mt);
-          const float al = fast_exp2(m_run - mn), be = fast_exp2(mt - mn);
-          const float l_new = fmaf(al, l_run, be * lt);
-          const float r = be / l_new;
-#pragma unroll
-          for (int j = 0; j < CPL; ++j) {
-            const float dlt = r * fmaf(-lt, x[j], pv[j]);
-            const float xn = x[j] + dlt;
-            sdd = fmaf(dlt, dlt, sdd); sad = fmaf(x[j], dlt, sad); saa = fmaf(x[j], x[j], saa); sbb = fmaf(xn, xn, sbb);
-            x[j] = xn;
-          }
-          m_run = mn; l_run = l_new;
-        } else {
-#pragma unroll
-          for (int j = 0; j < CPL; ++j) { saa = fmaf(x[j], x[j], saa); }
-          sbb = saa;
+        // how many consecutive steps have arrived (lane k looks at step t + k); the first one is waited for
+        while (!mbar_try_wait_cluster(bar(sm.mbox0 + (t - 1) % M), ((t - 1) / M) & 1)) {}
+        int n;
+        {
+          bool ok = lane == 0;
+          if (lane >= 1 && lane < kScanBatch && t + lane <= Tn && lane < M)
+            ok = mbar_test_wait(bar(sm.mbox0 + (t - 1 + lane) % M), ((t - 1 + lane) / M) & 1);
+          const uint32_t bits = __ballot_sync(0xffffffffu, ok);
+          n = __ffs(~bits) - 1;
+          n = n > kScanBatch ? kScanBatch : n;
         }
+        for (int k = 1; k < n; ++k)                          // every lane acquires the slots it is about to read
+          while (!mbar_try_wait_cluster(bar(sm.mbox0 + (t - 1 + k) % M), ((t - 1 + k) / M) & 1)) {}
+        const int t0 = t - 1;
+        const int fired = sc.batch(n, lane, p.tau, p.phi, p.patience,
+          [&](int k, bool live, float& mt, float& lt) {
+            const float* mb = mbox + static_cast<size_t>((t0 + k) % M) * G * ROWF + h * ROWF;
+            const float m_ = mb[0], l_ = mb[1];
+            mt = live ? m_ : kNegInf; lt = live ? l_ : 0.f;
+          },
+          [&](int k, bool live, float (&pv)[CPL]) {
+            const float* mb = mbox + static_cast<size_t>((t0 + k) % M) * G * ROWF + h * ROWF;
 #pragma unroll
-        for (int msk = LPH / 2; msk >= 1; msk >>= 1) {
-          sdd += __shfl_xor_sync(0xffffffffu, sdd, msk); sad += __shfl_xor_sync(0xffffffffu, sad, msk);
-          saa += __shfl_xor_sync(0xffffffffu, saa, msk); sbb += __shfl_xor_sync(0xffffffffu, sbb, msk);
-        }
-        // Eq. 2: d_scale = ||dx||; d_direction = 1 - cos(x_new, x_old), evaluated as
-        // (|a|^2 |d|^2 - (a.d)^2) / (|a||b| (|a||b| + a.b)) to avoid the cancellation in 1 - cos.
-        const float d_scale = sqrtf(sdd);
-        float d_dir = 1.f;                                   // zero norm => cos := 0 (R4)
-        if (saa > 0.f && sbb > 0.f) {
-          const float nanb = sqrtf(saa) * sqrtf(sbb);
-          const float ab = saa + sad;
-          if (ab > 0.f) d_dir = fmaxf(fmaf(saa, sdd, -sad * sad), 0.f) / (nanb * (nanb + ab));
-          else d_dir = 1.f - ab / nanb;
-        }
-        const bool stable_h = (d_scale < p.tau) && (d_dir < p.phi);          // strict (R5)
-        const bool stable = __all_sync(0xffffffffu, stable_h);               // AND over the group's heads (R2)
-        cnt = stable ? cnt + 1 : 0;                                          // Eq. 3
-        const bool fire = cnt >= p.patience;
-        // relaxed is enough: the value depends on this step's mailbox loads, so they have completed
-        if (lane < C) asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(mapa(a_ctrl, lane)), "r"(fire ? -t : t) : "memory");
-        if (fire) { t_stop = t; break; }
+            for (int j = 0; j < CPL; ++j) { const float v = mb[2 + sub + LPH * j]; pv[j] = live ? v : 0.f; }
+          });
+        __syncwarp();
+        const int t_last = fired >= 0 ? t + fired : t + n - 1;
+        // relaxed is enough: the value depends on the mailbox loads of these steps, so they have completed
+        if (lane < C) asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(mapa(a_ctrl, lane)), "r"(fired >= 0 ? -t_last : t_last) : "memory");
+        if (fired >= 0) { t_stop = t_last; break; }
+        t += n;
       }
       if (lane == 0) p.stop_block[group] = t_stop ? t_stop : Tn;             // t* (R9)
     } else {
