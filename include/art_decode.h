@@ -111,6 +111,10 @@ typedef struct art_thresholds {
  *                   call zeroes what it needs), may be NULL otherwise
  *
  * seq_lens[b] == 0 or an empty list gives a zero output row and stop_block 0.
+ * Reproducibility: stop_block is bit-deterministic for every schedule.  `out` is bit-reproducible when steps are
+ * dealt statically (clusters of 1 or > 4, ART-off); when the CTAs of a cluster claim steps at run time (ART-on with
+ * clusters of 2-4, ART_SPLIT_DYNAMIC) the order in which partial states are merged depends on the run and `out`
+ * agrees to fp32 rounding (<= 1e-5 relative) between runs.
  * Device-side contents (page ids in range, list entries valid) are not validated.
  */
 int art_decode_attention(const art_desc_t* desc, const void* q, const void* k_cache,

@@ -203,8 +203,10 @@ __device__ __forceinline__ void combine_group(const Params& p, const WsView& w, 
   for (int o = tid; o < G * kD; o += nthreads) {
     const int h = o / kD;
     float mx = kNegInf;
+#pragma unroll 4
     for (int s = 0; s < ns; ++s) mx = fmaxf(mx, __ldcg(part + s * w.part_floats + G * kD + h));
     float a = 0.f, l = 0.f;
+#pragma unroll 4                                               // four slots' loads in flight together
     for (int s = 0; s < ns; ++s) {
       const float* ps = part + s * w.part_floats;
       const float mc = __ldcg(ps + G * kD + h);
