@@ -93,6 +93,8 @@ def test_any_cluster_size_bf16(split):
 def test_layouts_agree(layout):
     w = small(3, sub="a", layout=layout, recency_decay=(0.2, 1.0))
     check(w, tau=1e-3, split=2)
+    check(w, tau=1e-3, split=-1)                # the dynamic scheduler reads the same tensor maps
+    check(w, art_on=False, split=-1)
 
 
 @pytest.mark.parametrize("G", [1, 2, 4, 8])
@@ -257,7 +259,7 @@ def test_host_entry_point():
 
 # ------------------------------------------------------------------ BASELINE-size configs, sampled groups
 
-FULL = [(1, "a", ""), (1, "a", "R"), (1, "a", "Rdyn"), (4, "a", "Rdyn"), (3, "a", ""), (3, "b", ""), (2, "a", ""), (2, "a", "R"), (3, "a", "R"), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
+FULL = [(1, "a", ""), (1, "a", "R"), (1, "a", "Rdyn"), (4, "a", "Rdyn"), (3, "a", "Rdyn"), (2, "a", "Rdyn"), (3, "a", ""), (3, "b", ""), (2, "a", ""), (2, "a", "R"), (3, "a", "R"), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
 
 
 @pytest.mark.parametrize("index,sub,variant", FULL)
