@@ -18,8 +18,10 @@
  * AND over heads, sink block first, zero-norm => d_direction = 1, strict '<') are
  * listed in DESIGN.md, "Readings".
  *
- * All functions are re-entrant; the library keeps no global mutable state, never
- * allocates or frees device memory, and never retains a pointer after returning.
+ * All functions are re-entrant; the library never allocates or frees device memory and never dereferences a
+ * pointer after returning.  Its only global state are three mutex-guarded host-side caches of values that are
+ * pure functions of their keys (kernel attributes already set, cluster occupancy, the last few tensor maps
+ * keyed by cache base pointer / layout / Hkv).
  * Nothing here falls back to the CPU: on a device that is not sm_100 the calls
  * return ART_ERR_ARCH.
  */
@@ -138,7 +140,8 @@ int art_decode_attention_off(const art_desc_t* desc, const void* q, const void* 
  * eligible_blocks, eligible_counts, seq_lens) are HOST buffers (pinned for async
  * copies), copied to the device inside the call; out and stop_block are HOST buffers
  * filled before the call returns (the call synchronises the stream).  The KV caches
- * are decode STATE and stay DEVICE pointers.  desc->eligible_counts is then a HOST
+ * are decode STATE and stay DEVICE pointers.  If out / stop_block are pinned (device-accessible) the kernel writes
+ * them directly, otherwise they are staged in the workspace and copied back.  desc->eligible_counts is then a HOST
  * pointer; desc->blocks_loaded must be NULL.  `thresholds == NULL` selects ART-off.
  * `workspace` is DEVICE scratch of at least art_workspace_bytes(desc).
  */

@@ -25,8 +25,26 @@ static void set_cluster_attr(cudaLaunchAttribute* attr, int C) {
   attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
 }
 
+template <typename Kern> static cudaError_t prepare_kernel_uncached(Kern kern, int C, uint32_t smem_bytes);
+// The attribute calls cost a few microseconds each on the host; they are idempotent per (device, kernel, shared
+// memory size, cluster size class), so they are made once and remembered.
 template <typename Kern>
 static cudaError_t prepare_kernel(Kern kern, int C, uint32_t smem_bytes) {
+  static std::mutex mu;
+  static std::map<std::array<uintptr_t, 4>, bool> done;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
+  const std::array<uintptr_t, 4> key = {static_cast<uintptr_t>(dev), reinterpret_cast<uintptr_t>(kern), smem_bytes, static_cast<uintptr_t>(C > 8)};
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    if (done.count(key)) return cudaSuccess;
+  }
+  cudaError_t e = prepare_kernel_uncached(kern, C, smem_bytes);
+  if (e == cudaSuccess) { std::lock_guard<std::mutex> lock(mu); done[key] = true; }
+  return e;
+}
+template <typename Kern>
+static cudaError_t prepare_kernel_uncached(Kern kern, int C, uint32_t smem_bytes) {
   cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes));
   if (e != cudaSuccess) return e;
   // two CTAs per SM need the whole unified L1/shared array configured as shared memory
@@ -101,7 +119,26 @@ static EncodeTiledFn encode_tiled_fn() {
 //   HND cache[page][head][token][d]:  dims (128, 64 tokens, page*Hkv + head)
 //   NHD cache[page][token][head][d]:  dims (128, Hkv, page*64 + token)
 // The outermost extent is not known to the ABI (the cache is the caller's); it is set to 2^30.
+static bool encode_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv);
+// Encoding a tensor map is a driver call; a decode loop passes the same caches every step, so the last few maps
+// are remembered (keyed by base pointer, layout, Hkv: everything the map depends on).
 static bool make_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv) {
+  struct Entry { const void* base; int layout, Hkv; CUtensorMap tm; };
+  static std::mutex mu;
+  static Entry cache[8];
+  static int n = 0, next = 0;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    for (int i = 0; i < n; ++i)
+      if (cache[i].base == base && cache[i].layout == layout && cache[i].Hkv == Hkv) { *tm = cache[i].tm; return true; }
+  }
+  if (!encode_cache_map(tm, base, layout, Hkv)) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  cache[next] = Entry{base, layout, Hkv, *tm};
+  next = (next + 1) % 8; if (n < 8) ++n;
+  return true;
+}
+static bool encode_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
   cuuint64_t dims[3]; cuuint64_t strides[2]; cuuint32_t box[3]; cuuint32_t es[3] = {1, 1, 1};
@@ -286,9 +323,7 @@ static size_t ws_bytes_for(const art_desc_t* d) {
 template <typename Kern>
 static cudaError_t launch_ws(Kern kern, int grid, uint32_t smem_bytes, cudaStream_t stream, const Params& p,
                              const ws::WsView& v, const CUtensorMap& tmK, const CUtensorMap& tmV) {
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes));
-  if (e != cudaSuccess) return e;
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, static_cast<int>(cudaSharedmemCarveoutMaxShared));
+  cudaError_t e = prepare_kernel(kern, 1, smem_bytes);
   if (e != cudaSuccess) return e;
   kern<<<grid, tc::kThreads, smem_bytes, stream>>>(p, v, tmK, tmV);
   return cudaGetLastError();
@@ -451,13 +486,29 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
     ok &= cudaMemcpyAsync(ws + h.ec, desc->eligible_counts, B * Hkv * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
   }
   if (!ok) { cudaGetLastError(); return ART_ERR_CUDA; }
+  // Results: if the caller's buffers are pinned (device-accessible under UVA) the kernel writes them directly, which
+  // saves two copies on the critical path of a decode step; otherwise they are staged and copied back.
+  float* out_dev = reinterpret_cast<float*>(ws + h.out);
+  int32_t* stop_dev = reinterpret_cast<int32_t*>(ws + h.stop);
+  bool direct = false;
+  {
+    cudaPointerAttributes ao, as;
+    if (cudaPointerGetAttributes(&ao, out_host) == cudaSuccess && cudaPointerGetAttributes(&as, stop_block_host) == cudaSuccess &&
+        ao.type == cudaMemoryTypeHost && as.type == cudaMemoryTypeHost && ao.devicePointer && as.devicePointer) {
+      out_dev = static_cast<float*>(ao.devicePointer); stop_dev = static_cast<int32_t*>(as.devicePointer); direct = true;
+    } else {
+      cudaGetLastError();
+    }
+  }
   rc = art::run(desc, ws + h.q, k_cache, v_cache, reinterpret_cast<const int32_t*>(ws + h.bt),
                 reinterpret_cast<const int32_t*>(ws + h.el), reinterpret_cast<const int32_t*>(ws + h.ec),
-                reinterpret_cast<const int32_t*>(ws + h.sl), thresholds, reinterpret_cast<float*>(ws + h.out),
-                reinterpret_cast<int32_t*>(ws + h.stop), nullptr, ws + h.kws, h.total - h.kws, st);
+                reinterpret_cast<const int32_t*>(ws + h.sl), thresholds, out_dev, stop_dev, nullptr,
+                ws + h.kws, h.total - h.kws, st);
   if (rc != ART_OK) return rc;
-  ok &= cudaMemcpyAsync(out_host, ws + h.out, B * Hq * D * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
-  ok &= cudaMemcpyAsync(stop_block_host, ws + h.stop, B * Hkv * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  if (!direct) {
+    ok &= cudaMemcpyAsync(out_host, ws + h.out, B * Hq * D * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+    ok &= cudaMemcpyAsync(stop_block_host, ws + h.stop, B * Hkv * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  }
   ok &= cudaStreamSynchronize(st) == cudaSuccess;
   if (!ok) { cudaGetLastError(); return ART_ERR_CUDA; }
   return ART_OK;
