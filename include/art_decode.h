@@ -140,7 +140,8 @@ int art_decode_attention_off(const art_desc_t* desc, const void* q, const void* 
  * eligible_blocks, eligible_counts, seq_lens) are HOST buffers (pinned for async
  * copies), copied to the device inside the call; out and stop_block are HOST buffers
  * filled before the call returns (the call synchronises the stream).  The KV caches
- * are decode STATE and stay DEVICE pointers.  If out / stop_block are pinned (device-accessible) the kernel writes
+ * are decode STATE and stay DEVICE pointers.  Pinned inputs are gathered into the workspace by one small kernel
+ * (pageable ones by one copy each).  If out / stop_block are pinned (device-accessible) the kernel writes
  * them directly, otherwise they are staged in the workspace and copied back.  desc->eligible_counts is then a HOST
  * pointer; desc->blocks_loaded must be NULL.  `thresholds == NULL` selects ART-off.
  * `workspace` is DEVICE scratch of at least art_workspace_bytes(desc).

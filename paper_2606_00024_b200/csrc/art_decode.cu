@@ -405,6 +405,27 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   return ART_OK;
 }
 
+// ---- host entry point: one gather kernel instead of up to five small copies.  The per-step inputs (q, tables,
+// lists: ~100 KB) are read straight out of the caller's PINNED buffers over PCIe, 16 bytes per thread.
+struct StageSegs { const uint8_t* src[5]; uint8_t* dst[5]; uint32_t wide[5]; uint32_t first[6]; };   // first[i]: units before segment i; unit = 16 B (wide) or 4 B
+__global__ void __launch_bounds__(256) art_stage_inputs_kernel(const StageSegs sg) {
+  const uint32_t u = blockIdx.x * blockDim.x + threadIdx.x;
+  if (u >= sg.first[5]) return;
+  int i = 0;
+#pragma unroll
+  for (int k = 1; k < 5; ++k) i += (u >= sg.first[k]) ? 1 : 0;
+  const uint32_t off = u - sg.first[i];
+  if (sg.wide[i]) reinterpret_cast<uint4*>(sg.dst[i])[off] = reinterpret_cast<const uint4*>(sg.src[i])[off];
+  else reinterpret_cast<uint32_t*>(sg.dst[i])[off] = reinterpret_cast<const uint32_t*>(sg.src[i])[off];
+}
+
+// device-accessible alias of a pinned host buffer (nullptr if the buffer is pageable or unknown to the runtime)
+static const uint8_t* pinned_alias(const void* host) {
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, host) != cudaSuccess) { cudaGetLastError(); return nullptr; }
+  return (a.type == cudaMemoryTypeHost && a.devicePointer) ? static_cast<const uint8_t*>(a.devicePointer) : nullptr;
+}
+
 }  // namespace art
 
 // ----------------------------------------------------------------------------- C ABI
@@ -478,12 +499,35 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
   const size_t B = desc->batch, Hq = desc->num_q_heads, Hkv = desc->num_kv_heads, D = desc->head_dim;
   if (B == 0) return ART_OK;
   bool ok = true;
-  ok &= cudaMemcpyAsync(ws + h.q, q_host, B * Hq * D * esz, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  ok &= cudaMemcpyAsync(ws + h.bt, block_table_host, B * static_cast<size_t>(desc->max_blocks_per_seq) * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  ok &= cudaMemcpyAsync(ws + h.sl, seq_lens_host, B * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  if (desc->policy == ART_POLICY_LIST) {
-    ok &= cudaMemcpyAsync(ws + h.el, eligible_blocks_host, B * Hkv * static_cast<size_t>(desc->max_eligible) * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
-    ok &= cudaMemcpyAsync(ws + h.ec, desc->eligible_counts, B * Hkv * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  {
+    const bool list = desc->policy == ART_POLICY_LIST;
+    const void* srcs[5] = {q_host, block_table_host, seq_lens_host, list ? eligible_blocks_host : nullptr, list ? desc->eligible_counts : nullptr};
+    const size_t offs[5] = {h.q, h.bt, h.sl, h.el, h.ec};
+    const size_t bytes[5] = {B * Hq * D * esz, B * static_cast<size_t>(desc->max_blocks_per_seq) * 4, B * 4,
+                             list ? B * Hkv * static_cast<size_t>(desc->max_eligible) * 4 : 0, list ? B * Hkv * 4 : 0};
+    // gather with one kernel when every buffer is pinned (16 bytes per thread where address and size allow it, else
+    // 4 bytes: every size here is a multiple of 4), else fall back to one copy per buffer
+    art::StageSegs sg = {};
+    bool gather = true;
+    uint32_t total = 0;
+    for (int i = 0; i < 5; ++i) {
+      sg.first[i] = total;
+      sg.dst[i] = ws + offs[i]; sg.src[i] = nullptr; sg.wide[i] = 0;
+      if (bytes[i] == 0) continue;
+      const uint8_t* alias = art::pinned_alias(srcs[i]);
+      if (!alias || (reinterpret_cast<uintptr_t>(alias) & 3u)) { gather = false; break; }
+      sg.src[i] = alias;
+      sg.wide[i] = (!(reinterpret_cast<uintptr_t>(alias) & 15u) && !(bytes[i] & 15u)) ? 1u : 0u;
+      total += static_cast<uint32_t>(bytes[i] / (sg.wide[i] ? 16 : 4));
+    }
+    sg.first[5] = total;
+    if (gather && total > 0) {
+      art::art_stage_inputs_kernel<<<(total + 255) / 256, 256, 0, st>>>(sg);
+      ok &= cudaGetLastError() == cudaSuccess;
+    } else {
+      for (int i = 0; i < 5; ++i)
+        if (bytes[i]) ok &= cudaMemcpyAsync(ws + offs[i], srcs[i], bytes[i], cudaMemcpyHostToDevice, st) == cudaSuccess;
+    }
   }
   if (!ok) { cudaGetLastError(); return ART_ERR_CUDA; }
   // Results: if the caller's buffers are pinned (device-accessible under UVA) the kernel writes them directly, which

@@ -255,6 +255,14 @@ def test_host_entry_point():
                                 w.eligible_blocks.pin_memory(), w.seq_lens.pin_memory(), None, out, stop, ws)
     o_dev, s_dev, _ = a.run_workload(wc, art=False)
     assert close(out, o_dev.cpu()) and torch.equal(stop, s_dev.cpu())
+    # pageable (not pinned) host buffers take the copy path instead of the gather kernel / direct output writes
+    out2 = torch.empty_like(out_p := torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32))
+    stop2 = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32)
+    desc2 = a.make_desc(w, eligible_counts=w.eligible_counts)
+    a.art_decode_attention_host(desc2, w.q, wc.k_cache, wc.v_cache, w.block_table, w.eligible_blocks, w.seq_lens, th,
+                                out2, stop2, ws)
+    o_dev, s_dev, _ = a.run_workload(wc, tau=1e-3)
+    assert close(out2, o_dev.cpu()) and torch.equal(stop2, s_dev.cpu())
 
 
 # ------------------------------------------------------------------ BASELINE-size configs, sampled groups
