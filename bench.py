@@ -377,7 +377,8 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
-                    help="time ONLY this arm of configs[1] (short command for ncu captures; prints a small JSON line)")
+                    help="time ONLY this arm of one config (short command for ncu captures; prints a small JSON line)")
+    ap.add_argument("--config", default="1a", help="config for --arm: index + sub, e.g. 1a, 2a, 3a, 3b, 4a, 0a")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "art" else args.warmup
 
@@ -409,6 +410,17 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         barrier = dist.barrier
     dev = torch.device("cuda", local)
+
+    if args.arm and args.config != "1a":
+        idx, sub = int(args.config[0]), args.config[1:] or "a"
+        wa = gen.config(idx, sub=sub, device=dev, variant="R" if args.arm.startswith("R_") else "")
+        torch.cuda.synchronize()
+        kw = {"patience": art.ART_PATIENCE_INF} if args.arm == "pinf" else {}
+        sp = args.split if wa.dtype == torch.bfloat16 else 0
+        r = measure(art, wa, args.steps, args.warmup, None, art_on=args.arm not in ("off", "R_off"), split=sp, **kw)
+        r.update(arm=args.arm, config=wa.name, split=sp or art.art_query_split(art.make_desc(wa), args.arm not in ("off", "R_off")))
+        print(json.dumps(r), flush=True)
+        return
 
     # configs[1]; every rank its own batch (seed offset), no exchange between ranks
     w = gen.config(1, device=dev, seed=rank_seed(rank))
