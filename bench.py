@@ -82,7 +82,7 @@ class ClockSampler:
                         self.reasons.add(name)
             except Exception:
                 pass
-            time.sleep(0.02)
+            time.sleep(0.001)                 # the timed region is ~10 ms: sample as fast as NVML answers
 
     def __enter__(self):
         self._t.start(); return self
