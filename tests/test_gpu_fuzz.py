@@ -1,0 +1,43 @@
+"""-m gpu: seeded random shapes / policies / thresholds / schedules against the fp64 oracle.  Every case goes
+through the same check as the hand-written parity tests (stop blocks exact on non-fragile groups, outputs within
+tolerance, loaded >= processed)."""
+import numpy as np
+import pytest
+import torch
+
+from workloads import generators as gen
+from test_gpu_parity import check
+
+pytestmark = pytest.mark.gpu
+
+
+def random_case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    bf16 = bool(rng.integers(0, 4) > 0)                      # mostly the bf16 tensor-core path
+    dtype, d = (torch.bfloat16, 128) if bf16 else (torch.float32, 64)
+    G = int(rng.choice([1, 2, 4, 8]))
+    Hkv = int(rng.integers(1, 4))
+    B = int(rng.integers(1, 5))
+    lens = [int(rng.choice([0, 1, 63, 64, 65, int(rng.integers(100, 6000))], p=[.05, .05, .05, .05, .05, .75])) for _ in range(B)]
+    policy = int(rng.choice([gen.POLICY_DENSE, gen.POLICY_SINK_WINDOW, gen.POLICY_LIST]))
+    kw = {}
+    if policy == gen.POLICY_SINK_WINDOW:
+        kw = dict(sink_tokens=int(rng.choice([0, 4, 70, 200])), window_tokens=int(rng.choice([0, 100, 1000, 4096])))
+    elif policy == gen.POLICY_LIST:
+        kw = dict(topk_blocks=int(rng.integers(1, 40)))
+    layout = int(rng.choice([gen.LAYOUT_HND, gen.LAYOUT_NHD])) if bf16 else gen.LAYOUT_HND
+    w = gen.make_workload(f"fuzz{seed}", seed=7000 + seed, batch=B, num_q_heads=G * Hkv, num_kv_heads=Hkv, head_dim=d,
+                          seq_lens=lens, dtype=dtype, policy=policy, layout=layout,
+                          recency_decay=(0.05, 1.0) if rng.integers(0, 4) else None,
+                          planted_frac=0.01 if rng.integers(0, 2) else 0.0, **kw)
+    th = dict(tau=float(rng.choice([1e-5, 3e-4, 1e-3, 5e-3])), phi=float(rng.choice([1e-3, 1e-2, float("inf")])),
+              patience=int(rng.choice([1, 2, 5, 7])), probe_dim=int(rng.choice([32, 32, 0])))
+    splits = [0, 1, 2, 4, 8, 16] + ([3, 5, -1, -1] if bf16 else [])
+    return w, th, int(rng.choice(splits))
+
+
+@pytest.mark.parametrize("seed", range(48))
+def test_random_case(seed):
+    w, th, split = random_case(seed)
+    check(w, split=split, **th)
+    check(w, art_on=False, split=split)
