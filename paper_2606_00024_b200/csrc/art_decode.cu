@@ -6,6 +6,8 @@
 //   art_decode_simt.cuh  fp32 KV, head_dim 64:  TMA bulk loads, CUDA-core FMAs (1e-5 tolerance rules out TF32)
 // The ART-off entry point is the same kernel template with the detector compiled out.
 #include <array>
+#include <cstdio>
+#include <cstdlib>
 #include <map>
 #include <mutex>
 #include <utility>
@@ -26,21 +28,23 @@ static void set_cluster_attr(cudaLaunchAttribute* attr, int C) {
 }
 
 template <typename Kern> static cudaError_t prepare_kernel_uncached(Kern kern, int C, uint32_t smem_bytes);
-// The attribute calls cost a few microseconds each on the host; they are idempotent per (device, kernel, shared
-// memory size, cluster size class), so they are made once and remembered.
+// The attribute calls cost a few microseconds each on the host.  They are per-function state, so what has been set
+// is remembered per (device, kernel): the dynamic shared memory limit only ever grows (a larger limit than a launch
+// needs is harmless), the carveout preference and the non-portable cluster size are set once.
 template <typename Kern>
 static cudaError_t prepare_kernel(Kern kern, int C, uint32_t smem_bytes) {
+  struct State { uint32_t smem = 0; bool nonportable = false; };
   static std::mutex mu;
-  static std::map<std::array<uintptr_t, 4>, bool> done;
+  static std::map<std::array<uintptr_t, 2>, State> done;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
-  const std::array<uintptr_t, 4> key = {static_cast<uintptr_t>(dev), reinterpret_cast<uintptr_t>(kern), smem_bytes, static_cast<uintptr_t>(C > 8)};
-  {
-    std::lock_guard<std::mutex> lock(mu);
-    if (done.count(key)) return cudaSuccess;
-  }
-  cudaError_t e = prepare_kernel_uncached(kern, C, smem_bytes);
-  if (e == cudaSuccess) { std::lock_guard<std::mutex> lock(mu); done[key] = true; }
+  const std::array<uintptr_t, 2> key = {static_cast<uintptr_t>(dev), reinterpret_cast<uintptr_t>(kern)};
+  std::lock_guard<std::mutex> lock(mu);
+  State& st = done[key];
+  if (st.smem >= smem_bytes && (C <= 8 || st.nonportable)) return cudaSuccess;
+  const uint32_t want = smem_bytes > st.smem ? smem_bytes : st.smem;
+  cudaError_t e = prepare_kernel_uncached(kern, C > 8 || st.nonportable ? 16 : 1, want);
+  if (e == cudaSuccess) { st.smem = want; st.nonportable = st.nonportable || C > 8; }
   return e;
 }
 template <typename Kern>

@@ -221,6 +221,18 @@ def test_error_codes_on_device():
     assert a.art_query_split(a.make_desc(w, split=-1), True) == 0   # dynamic scheduler: no fixed cluster
 
 
+def test_launch_shapes_can_alternate():
+    """Per-kernel launch attributes are cached on the host: going back to a larger shared-memory shape after a
+    smaller one must still launch (regression: the fuzz sweep found the limit left at the smaller value)."""
+    w = gen.config(0, variant="c")
+    for split in (16, 1, 16, 2, 8, 1, 4, 16):
+        check(w, split=split)
+        check(w, art_on=False, split=split)
+    wb = small(1, recency_decay=(0.2, 1.0))
+    for split in (8, 1, -1, 8, 3, 16, 1):
+        check(wb, split=split, tau=1e-3)
+
+
 def test_dynamic_scheduler_needs_workspace():
     a = art()
     w = small(1).to("cuda")
