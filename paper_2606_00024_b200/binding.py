@@ -116,7 +116,8 @@ _ws_cache = {}
 
 def _workspace_for(desc: ArtDesc, device) -> torch.Tensor:
     """Device scratch of art_workspace_bytes(desc), cached per device (grown on demand).  The library never
-    allocates; the caller (here: the binding, with torch) owns the memory."""
+    allocates; the caller (here: the binding, with torch) owns the memory.  One scratch per device: calls on
+    DIFFERENT streams that may overlap (dynamic scheduler, host entry point) must pass their own `workspace`."""
     need = max(art_workspace_bytes(desc), 256)
     key = (device.type, device.index)
     ws = _ws_cache.get(key)
