@@ -44,7 +44,7 @@ extern "C" {
 enum {
   ART_OK = 0,
   ART_ERR_NULL = -1,      /* a required pointer is NULL */
-  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G not in {1,2,4,8}, unsupported head_dim, block_tokens != 64,
+  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G = Hq / Hkv > 8, unsupported head_dim, block_tokens != 64,
                              negative sizes, policy/list mismatch, bad thresholds */
   ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128) */
   ART_ERR_ALIGN = -4,     /* q / k_cache / v_cache not 16-byte aligned */
@@ -65,7 +65,8 @@ enum { ART_POLICY_DENSE = 0,        /* all blocks, most recent first (PAPER.md:1
 typedef struct art_desc {
   int32_t batch;               /* B */
   int32_t num_q_heads;         /* Hq */
-  int32_t num_kv_heads;        /* Hkv; query head h uses KV head h / (Hq/Hkv) */
+  int32_t num_kv_heads;        /* Hkv; query head h uses KV head h / (Hq/Hkv); G = Hq / Hkv must be 1..8 (kernels are
+                                  built for 1, 2, 4, 8: other sizes run the next one up with padding heads) */
   int32_t head_dim;            /* d: 64 (F32) or 128 (BF16) */
   int32_t block_tokens;        /* must be 64 */
   int32_t dtype;               /* ART_DTYPE_* */

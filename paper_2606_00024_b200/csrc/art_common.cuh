@@ -32,6 +32,7 @@ struct Params {
   int32_t* stop_block;
   int32_t* blocks_loaded;
   int32_t batch, Hq, Hkv;
+  int32_t Gr;                                        // real heads per group (Hq / Hkv); kernels are built for the next power of two
   int32_t max_blocks, max_elig;
   int32_t policy, layout, sink, window;
   int64_t page_stride, head_stride, token_stride;   // bytes

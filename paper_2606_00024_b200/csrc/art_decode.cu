@@ -20,6 +20,9 @@ namespace art {
 
 // ----------------------------------------------------------------------------- host side
 
+// kernels are instantiated for 1, 2, 4, 8 heads per group; other group sizes run the next one up with padding heads
+static inline int padded_group(int g) { return g <= 1 ? 1 : (g <= 2 ? 2 : (g <= 4 ? 4 : 8)); }
+
 struct LaunchPlan { int C, stages, mslots; uint32_t smem; };
 
 static void set_cluster_attr(cudaLaunchAttribute* attr, int C) {
@@ -167,7 +170,7 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
   if (d->batch < 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->max_blocks_per_seq < 0) return ART_ERR_SHAPE;
   if (d->num_q_heads % d->num_kv_heads != 0) return ART_ERR_SHAPE;
   const int G = d->num_q_heads / d->num_kv_heads;
-  if (G != 1 && G != 2 && G != 4 && G != 8) return ART_ERR_SHAPE;
+  if (G > 8) return ART_ERR_SHAPE;
   if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
   if (d->dtype != ART_DTYPE_F32 && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (d->head_dim != 64 && d->head_dim != 128) return ART_ERR_SHAPE;
@@ -271,7 +274,7 @@ static int cluster_capacity(const art_desc_t* d, int G, int mode, int C, uint32_
 // group streams from the first cycle; never more CTAs than a group could have blocks.  The tensor-core
 // kernel takes any C (steps are dealt round-robin); the CUDA-core kernel's mailbox wants a power of two.
 static int choose_split(const art_desc_t* d, int mode, int* C_out) {
-  const int G = d->num_q_heads / d->num_kv_heads;
+  const int G = padded_group(d->num_q_heads / d->num_kv_heads);
   const int groups = d->batch * d->num_kv_heads;
   const bool art = mode != 0;
   const int PW = mode == 2 ? d->head_dim : 32;
@@ -319,8 +322,8 @@ static int sm_count() {
 
 // workspace the dynamically scheduled kernel needs (worst case over the probe widths)
 static size_t ws_bytes_for(const art_desc_t* d) {
-  if (d->dtype != ART_DTYPE_BF16 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads) return 0;
-  const int G = d->num_q_heads / d->num_kv_heads;
+  if (d->dtype != ART_DTYPE_BF16 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads || d->num_q_heads / d->num_kv_heads > 8) return 0;
+  const int G = padded_group(d->num_q_heads / d->num_kv_heads);
   return ws::make_ws_layout(d->batch * d->num_kv_heads, G, d->head_dim, true).total;
 }
 
@@ -339,7 +342,7 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
                cudaStream_t stream) {
   const int groups = d->batch * d->num_kv_heads;
   if (groups == 0) return ART_OK;
-  const int G = d->num_q_heads / d->num_kv_heads;
+  const int G = padded_group(d->num_q_heads / d->num_kv_heads);
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
@@ -353,7 +356,7 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   p.q = q; p.k = static_cast<const uint8_t*>(k); p.v = static_cast<const uint8_t*>(v);
   p.block_table = bt; p.elig = elig; p.elig_counts = elig_counts; p.seq_lens = sl;
   p.out = out; p.stop_block = stop; p.blocks_loaded = blocks_loaded;
-  p.batch = d->batch; p.Hq = d->num_q_heads; p.Hkv = d->num_kv_heads;
+  p.batch = d->batch; p.Hq = d->num_q_heads; p.Hkv = d->num_kv_heads; p.Gr = d->num_q_heads / d->num_kv_heads;
   p.max_blocks = d->max_blocks_per_seq; p.max_elig = d->max_eligible;
   p.policy = d->policy; p.layout = d->kv_layout; p.sink = d->sink_tokens; p.window = d->window_tokens;
   const int64_t row = kRowBytes;
@@ -569,8 +572,8 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
                     int32_t* eligible_counts, void* cuda_stream) {
   if (!d || !q || !k_cache || !block_table || !seq_lens || !block_scores || !eligible_blocks || !eligible_counts) return ART_ERR_NULL;
   if (d->batch < 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads) return ART_ERR_SHAPE;
-  const int G = d->num_q_heads / d->num_kv_heads;
-  if (G != 1 && G != 2 && G != 4 && G != 8) return ART_ERR_SHAPE;
+  if (d->num_q_heads / d->num_kv_heads > 8) return ART_ERR_SHAPE;
+  const int G = art::padded_group(d->num_q_heads / d->num_kv_heads);
   if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
   if (!((d->dtype == ART_DTYPE_F32 && d->head_dim == 64) || (d->dtype == ART_DTYPE_BF16 && d->head_dim == 128))) return ART_ERR_DTYPE;
   if (d->kv_layout != ART_LAYOUT_HND && d->kv_layout != ART_LAYOUT_NHD) return ART_ERR_SHAPE;
@@ -585,7 +588,7 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
 
   art::policy::ScoreParams sp = {};
   sp.q = q; sp.k = static_cast<const uint8_t*>(k_cache); sp.block_table = block_table; sp.seq_lens = seq_lens;
-  sp.scores = block_scores; sp.batch = d->batch; sp.Hq = d->num_q_heads; sp.Hkv = d->num_kv_heads;
+  sp.scores = block_scores; sp.batch = d->batch; sp.Hq = d->num_q_heads; sp.Hkv = d->num_kv_heads; sp.Gr = d->num_q_heads / d->num_kv_heads;
   sp.max_blocks = d->max_blocks_per_seq; sp.layout = d->kv_layout;
   const int64_t row = art::kRowBytes;
   if (d->kv_layout == ART_LAYOUT_HND) { sp.token_stride = row; sp.head_stride = row * art::kBlockTokens; sp.page_stride = sp.head_stride * d->num_kv_heads; }
@@ -614,8 +617,7 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
 int art_query_split(const art_desc_t* desc, int art_on) {
   if (!desc) return ART_ERR_NULL;
   if (desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->num_q_heads % desc->num_kv_heads) return ART_ERR_SHAPE;
-  const int G = desc->num_q_heads / desc->num_kv_heads;
-  if (G != 1 && G != 2 && G != 4 && G != 8) return ART_ERR_SHAPE;
+  if (desc->num_q_heads / desc->num_kv_heads > 8) return ART_ERR_SHAPE;
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;

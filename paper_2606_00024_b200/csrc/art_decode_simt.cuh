@@ -244,11 +244,11 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
     const int half = lane >> 4, c16 = lane & 15;
     float qreg[G][E16];                                      // this lane's 16-byte chunk of every head's q
     {
-      const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * G) * D + c16 * E16;
+      const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * D + c16 * E16;
 #pragma unroll
       for (int h = 0; h < G; ++h)
 #pragma unroll
-        for (int e = 0; e < E16; ++e) qreg[h][e] = to_float(qp[h * D + e]) * p.scale_log2;
+        for (int e = 0; e < E16; ++e) qreg[h][e] = (h < p.Gr) ? to_float(qp[h * D + e]) * p.scale_log2 : 0.f;   // padding heads: q = 0
     }
     float pend[G][E8], pend_m[G], pend_l[G];
     bool have_pend = false; int pend_t = 0;
@@ -422,7 +422,7 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
       // The leader's own steps do not arrive by themselves: the scan warp moves each of them from the summary
       // buffers into its mailbox slot first, then every step of the group is read from the mailbox alike.
       using Scan = ScanCore<G, PW>;
-      Scan sc; sc.init();
+      Scan sc; sc.init(); sc.g_real = p.Gr;
       int t = 1, t_stop = 0, own_next = 0;                   // own_next: next local iteration to move (step own_next * C + 1)
       while (t <= Tn) {
         while (own_next < n_c) {
@@ -540,7 +540,7 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
         a = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta[o]), c)), a);
         l = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta_l[h]), c)), l);
       }
-      p.out[(static_cast<int64_t>(b) * p.Hq + g * G) * D + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
+      if (h < p.Gr) p.out[(static_cast<int64_t>(b) * p.Hq + g * p.Gr) * D + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
     }
     if (tid == 0) {
       if (!ART) p.stop_block[group] = Tn;

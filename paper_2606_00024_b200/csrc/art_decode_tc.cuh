@@ -288,10 +288,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   }
   if (warp == kWarpMmaPV) tmem_alloc(a_tmem, kTmemCols);
   {
-    const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * G) * kD;
+    const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD;
     for (int idx = tid; idx < 8 * kD; idx += kThreads) {       // rows >= G: zeros (rows 8-15 alias, see kQLbo)
       const int row = idx / kD, dc = idx % kD;
-      const __nv_bfloat16 v = (row < G) ? qp[row * kD + dc] : __float2bfloat16_rn(0.f);
+      const __nv_bfloat16 v = (row < p.Gr) ? qp[row * kD + dc] : __float2bfloat16_rn(0.f);
       *reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + (dc >> 3) * kQLbo + row * 16 + (dc & 7) * 2) = v;
     }
     if (tid < 64) reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + 16 * kQLbo)[tid] = __float2bfloat16_rn(0.f);
@@ -651,7 +651,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     using Scan = ScanCore<G, PW>;
     constexpr int LPH = Scan::LPH, CPL = Scan::CPL;
     const int h = lane / LPH, sub = lane % LPH;
-    Scan sc; sc.init();
+    Scan sc; sc.init(); sc.g_real = p.Gr;
     TC_TRACE_INIT(trs, 2);
     const uint32_t mb_lane = sbase + sm.mbox + h * 4u;         // this lane's head column of a mailbox row block
     int t_stop = 0;
@@ -721,7 +721,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         a = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta[o]), c)), a);
         l = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta_l[h]), c)), l);
       }
-      p.out[(static_cast<int64_t>(b) * p.Hq + g * G) * kD + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
+      if (h < p.Gr) p.out[(static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
     }
     if (tid == 0) {
       if (!ART) p.stop_block[group] = Tn;

@@ -199,8 +199,8 @@ __device__ __forceinline__ void combine_group(const Params& p, const WsView& w, 
   ns = ns > static_cast<int>(w.Wmax) ? static_cast<int>(w.Wmax) : ns;
   const float* part = reinterpret_cast<const float*>(w.base + w.off_part) + static_cast<size_t>(group) * w.Wmax * w.part_floats;
   const int b = group / p.Hkv, g = group % p.Hkv;
-  float* out = p.out + (static_cast<int64_t>(b) * p.Hq + g * G) * kD;
-  for (int o = tid; o < G * kD; o += nthreads) {
+  float* out = p.out + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD;
+  for (int o = tid; o < p.Gr * kD; o += nthreads) {
     const int h = o / kD;
     float mx = kNegInf;
 #pragma unroll 4

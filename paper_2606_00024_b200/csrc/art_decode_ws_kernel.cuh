@@ -191,8 +191,8 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
         mbar_wait(bar(sm.empty0 + last_marker % S), static_cast<uint32_t>((last_marker / S) & 1));
       {
         const uint4* qp = reinterpret_cast<const uint4*>(reinterpret_cast<const __nv_bfloat16*>(p.q) +
-                                                         (static_cast<int64_t>(b) * p.Hq + g * G) * kD);
-        for (int idx = lane; idx < G * 16; idx += 32) {        // 16-byte chunk (row, 8 d) -> K-major core matrices
+                                                         (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD);
+        for (int idx = lane; idx < p.Gr * 16; idx += 32) {        // 16-byte chunk (row, 8 d) -> K-major core matrices
           const int row = idx >> 4, dc = idx & 15;
           *reinterpret_cast<uint4*>(smem + sm.qb + dc * kQLbo + row * 16) = qp[row * 16 + dc];
         }
@@ -521,8 +521,8 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
       const Trav tr = make_trav(p, b, g, p.seq_lens[b]);
       const int Tn = tr.T;
       if (Tn == 0) {                                          // empty group: zero row, stop_block 0
-        float* out = p.out + (static_cast<int64_t>(b) * p.Hq + g * G) * kD;
-        for (int o = lane; o < G * kD; o += 32) out[o] = 0.f;
+        float* out = p.out + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD;
+        for (int o = lane; o < p.Gr * kD; o += 32) out[o] = 0.f;
       }
       if (lane == 0) {
         if (!ART || Tn == 0) p.stop_block[grp] = Tn;
@@ -531,7 +531,7 @@ art_decode_ws_kernel(const Params p, const WsView w, const __grid_constant__ CUt
       }
       if constexpr (ART) {
         if (Tn == 0) continue;
-        Scan sc; sc.init();
+        Scan sc; sc.init(); sc.g_real = p.Gr;
         int* c_ctrl = ctl(grp) + C_CTRL;
         const uint8_t* pay = reinterpret_cast<const uint8_t*>(pay_base + static_cast<size_t>(grp) * M * kPayFloats);
         // The mailbox is consumed in aligned blocks of kScanBatch steps through two staging halves: while block b

@@ -21,7 +21,7 @@ struct ScoreParams {
   const int32_t* block_table;
   const int32_t* seq_lens;
   float* scores;                               // [B, Hkv, max_blocks]
-  int32_t batch, Hq, Hkv, max_blocks, layout;
+  int32_t batch, Hq, Hkv, Gr, max_blocks, layout;   // Gr: real heads per group (the template G is its power-of-two ceiling)
   int64_t page_stride, head_stride, token_stride;   // bytes
 };
 
@@ -61,9 +61,10 @@ __global__ void __launch_bounds__(kScoreWarps * 32) art_block_scores_kernel(cons
   float qs[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) qs[e] = 0.f;
-  const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * G) * D;
+  const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * D;
 #pragma unroll
   for (int h = 0; h < G; ++h) {
+    if (h >= p.Gr) break;
     float f[E];
     Elem<T>::unpack(*reinterpret_cast<const uint4*>(qp + h * D + chunk * E), f);
 #pragma unroll
@@ -84,7 +85,7 @@ __global__ void __launch_bounds__(kScoreWarps * 32) art_block_scores_kernel(cons
   }
 #pragma unroll
   for (int m = 16; m >= 1; m >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, m);
-  if (lane == 0) *out = acc / static_cast<float>(G * n_valid) + 0.f;   // + 0: -0 and +0 are the same score
+  if (lane == 0) *out = acc / static_cast<float>(p.Gr * n_valid) + 0.f;   // + 0: -0 and +0 are the same score
 }
 
 struct TopkParams {

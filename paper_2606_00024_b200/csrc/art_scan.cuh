@@ -33,6 +33,7 @@ struct ScanCore {
   float m_run, l_run;       // running reference exponent (log2 domain) and A_t relative to it
   float x[CPL];             // probe of the normalised output, x^(t)
   int cnt;                  // c^(t)
+  int g_real = G;           // heads that exist; padding heads (q = 0) never hold the decision back
 
   __device__ __forceinline__ void init() {
     m_run = kNegInf; l_run = 0.f; cnt = 0;                // c^(0) = 0 (Alg. 1 l.2)
@@ -133,7 +134,7 @@ struct ScanCore {
     constexpr int KH = kh<NB>();
     uint32_t votes[KH];
 #pragma unroll
-    for (int j = 0; j < KH; ++j) votes[j] = __ballot_sync(0xffffffffu, stable_head(s[j], tau, phi));
+    for (int j = 0; j < KH; ++j) votes[j] = __ballot_sync(0xffffffffu, stable_head(s[j], tau, phi) || (lane / LPH) >= g_real);
     // far from convergence no step of the batch is stable: the counter is simply back at 0 (Eq. 3)
     bool any = false;
 #pragma unroll

@@ -57,7 +57,7 @@ def test_argument_validation_happens_before_cuda(art):
     """Fake (never dereferenced) pointers: every error below is decided on the host."""
     assert _call_off(art, good_desc(art), q=None) == -1                      # ART_ERR_NULL
     assert _call_off(art, good_desc(art, num_q_heads=7)) == -2               # Hq % Hkv
-    assert _call_off(art, good_desc(art, num_q_heads=32, num_kv_heads=2)) == -2   # G = 16 unsupported
+    assert _call_off(art, good_desc(art, num_q_heads=32, num_kv_heads=2)) == -2   # G = 16 unsupported (1..8 are)
     assert _call_off(art, good_desc(art, block_tokens=32)) == -2
     assert _call_off(art, good_desc(art, head_dim=96)) == -2
     assert _call_off(art, good_desc(art, head_dim=64)) == -3                 # bf16 d=64 not built

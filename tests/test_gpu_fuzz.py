@@ -15,7 +15,7 @@ def random_case(seed):
     rng = np.random.default_rng(1000 + seed)
     bf16 = bool(rng.integers(0, 4) > 0)                      # mostly the bf16 tensor-core path
     dtype, d = (torch.bfloat16, 128) if bf16 else (torch.float32, 64)
-    G = int(rng.choice([1, 2, 4, 8]))
+    G = int(rng.choice([1, 2, 3, 4, 5, 6, 7, 8]))
     Hkv = int(rng.integers(1, 4))
     B = int(rng.integers(1, 5))
     lens = [int(rng.choice([0, 1, 63, 64, 65, int(rng.integers(100, 6000))], p=[.05, .05, .05, .05, .05, .75])) for _ in range(B)]

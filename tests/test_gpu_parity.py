@@ -132,6 +132,22 @@ def test_dynamic_scheduler_stop_blocks_equal_cluster_kernel():
         assert (o - ref_o).abs().max() <= 1e-5 * ref_o.abs().max()
 
 
+@pytest.mark.parametrize("G", [3, 5, 6, 7])
+@pytest.mark.parametrize("dtype", [torch.float32, torch.bfloat16])
+def test_group_sizes_that_are_not_powers_of_two(G, dtype):
+    """Kernels are instantiated for 1, 2, 4, 8 heads per group; 3, 5, 6, 7 run the next one up with padding heads
+    (q = 0) that are neither written nor allowed to hold the termination decision back."""
+    d = 64 if dtype == torch.float32 else 128
+    w = gen.make_workload("g", seed=50 + G, batch=3, num_q_heads=2 * G, num_kv_heads=2, head_dim=d,
+                          seq_lens=[1000, 64, 3111], dtype=dtype, recency_decay=(0.3, 1.0))
+    check(w, tau=1e-3, split=2, expect_fired=True)
+    check(w, art_on=False, split=4)
+    check(w, tau=2e-3, probe_dim=0, split=1)
+    if dtype == torch.bfloat16:
+        check(w, tau=1e-3, split=-1, expect_fired=True)
+        check(w, art_on=False, split=-1)
+
+
 def test_full_probe():
     """probe_dim = 0: the detector sees all d coordinates."""
     for dtype, d in ((torch.bfloat16, 128), (torch.float32, 64)):

@@ -60,7 +60,7 @@ def check_policy(w, top_k):
     return s, l, c
 
 
-@pytest.mark.parametrize("G", [1, 2, 4, 8])
+@pytest.mark.parametrize("G", [1, 2, 3, 4, 6, 8])
 @pytest.mark.parametrize("dtype,layout", [(torch.bfloat16, gen.LAYOUT_HND), (torch.bfloat16, gen.LAYOUT_NHD),
                                           (torch.float32, gen.LAYOUT_HND)])
 def test_scores_and_lists_match_oracle(G, dtype, layout):
