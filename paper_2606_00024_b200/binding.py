@@ -178,7 +178,7 @@ def art_topk_blocks(desc, q, k_cache, block_table, seq_lens, top_k, block_scores
 
 # ------------------------------------------------------------------ convenience (argument marshalling only)
 
-def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None) -> ArtDesc:
+def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None, sm_scale: float = 0.0) -> ArtDesc:
     """Fill an art_desc_t from a workload-like object (fields as in workloads.generators.Workload)."""
     ec = eligible_counts if eligible_counts is not None else w.eligible_counts
     return ArtDesc(
@@ -187,20 +187,20 @@ def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None) ->
         kv_layout=w.layout, policy=w.policy, max_blocks_per_seq=int(w.block_table.shape[1]),
         sink_tokens=w.sink_tokens, window_tokens=w.window_tokens,
         max_eligible=0 if w.eligible_blocks is None else int(w.eligible_blocks.shape[2]),
-        sm_scale=0.0, split=split,
+        sm_scale=sm_scale, split=split,
         eligible_counts=None if ec is None else ec.data_ptr(),
         blocks_loaded=None if blocks_loaded is None else blocks_loaded.data_ptr())
 
 
 def run_workload(w, *, art: bool = True, split: int = 0, tau=None, phi=None, patience=None, probe_dim=None,
-                 want_loaded: bool = False, stream=None):
+                 want_loaded: bool = False, stream=None, sm_scale: float = 0.0):
     """Allocate outputs and run one decode step on a CUDA-resident workload.
     Returns (out [B,Hq,d] fp32, stop_block [B,Hkv] int32, blocks_loaded or None)."""
     dev = w.q.device
     out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32, device=dev)
     stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev)
     loaded = torch.zeros((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev) if want_loaded else None
-    desc = make_desc(w, split=split, blocks_loaded=loaded)
+    desc = make_desc(w, split=split, blocks_loaded=loaded, sm_scale=sm_scale)
     if art:
         th = ArtThresholds(tau=w.tau if tau is None else tau, phi=w.phi if phi is None else phi,
                            patience=w.patience if patience is None else patience,

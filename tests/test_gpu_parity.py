@@ -237,6 +237,20 @@ def test_error_codes_on_device():
     assert a.art_query_split(a.make_desc(w, split=-1), True) == 0   # dynamic scheduler: no fixed cluster
 
 
+def test_sm_scale_override():
+    """desc.sm_scale > 0 replaces 1/sqrt(d) (Eq. 1, R11) on every path."""
+    a = art()
+    for w, split in ((small(1, recency_decay=(0.2, 1.0)), 2), (small(1, recency_decay=(0.2, 1.0)), -1), (gen.config(0, variant="c"), 4)):
+        wc = w.to("cuda")
+        scale = float(np.float32(0.05))
+        for art_on in (True, False):
+            out, stop, _ = a.run_workload(wc, art=art_on, split=split, tau=1e-3, sm_scale=scale)
+            rep = compare(w, out, stop, art=art_on, oracle_over={"tau": f32(1e-3), "sm_scale": scale})
+            assert rep.stop_mismatch_nonfragile == 0 and rep.max_rel_err <= OUT_TOL[w.dtype], rep
+        out_d, _, _ = a.run_workload(wc, art=False, split=split)
+        assert (out - out_d).abs().max() > 1e-3                  # the override really changed the result
+
+
 def test_launch_shapes_can_alternate():
     """Per-kernel launch attributes are cached on the host: going back to a larger shared-memory shape after a
     smaller one must still launch (regression: the fuzz sweep found the limit left at the smaller value)."""
