@@ -75,6 +75,10 @@ def test_argument_validation_happens_before_cuda(art):
     rc = lib.art_decode_attention(C.byref(good_desc(art)), vp(16), vp(32), vp(48), vp(64), None, vp(80), C.byref(th),
                                   vp(96), vp(112), None, 0, None)
     assert rc == -2                                                          # patience < 1
+    th = art.ArtThresholds(tau=float("nan"), phi=1e-3, patience=5, probe_dim=32)
+    rc = lib.art_decode_attention(C.byref(good_desc(art)), vp(16), vp(32), vp(48), vp(64), None, vp(80), C.byref(th),
+                                  vp(96), vp(112), None, 0, None)
+    assert rc == -2                                                          # NaN threshold
     th = art.ArtThresholds(tau=1e-5, phi=1e-3, patience=5, probe_dim=48)
     rc = lib.art_decode_attention(C.byref(good_desc(art)), vp(16), vp(32), vp(48), vp(64), None, vp(80), C.byref(th),
                                   vp(96), vp(112), None, 0, None)

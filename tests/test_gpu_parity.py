@@ -251,6 +251,21 @@ def test_sm_scale_override():
         assert (out - out_d).abs().max() > 1e-3                  # the override really changed the result
 
 
+def test_side_stream_and_probe_dim_alias():
+    """The call enqueues on the stream it is given; probe_dim == head_dim means the same as 0 (all coordinates)."""
+    a = art()
+    w = small(1, recency_decay=(0.2, 1.0)); wc = w.to("cuda")
+    ref_o, ref_s, _ = a.run_workload(wc, tau=2e-3, probe_dim=0, split=1)
+    torch.cuda.synchronize()
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        o, s, _ = a.run_workload(wc, tau=2e-3, probe_dim=128, split=1)
+        o2, s2, _ = a.run_workload(wc, tau=2e-3, probe_dim=128, split=-1)
+    side.synchronize()
+    assert torch.equal(s, ref_s) and torch.equal(o, ref_o)
+    assert torch.equal(s2, ref_s) and (o2 - ref_o).abs().max() <= 1e-5 * ref_o.abs().max()
+
+
 def test_launch_shapes_can_alternate():
     """Per-kernel launch attributes are cached on the host: going back to a larger shared-memory shape after a
     smaller one must still launch (regression: the fuzz sweep found the limit left at the smaller value)."""
