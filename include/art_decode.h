@@ -48,7 +48,8 @@ enum {
                              negative sizes, policy/list mismatch, bad thresholds */
   ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128) */
   ART_ERR_ALIGN = -4,     /* q / k_cache / v_cache not 16-byte aligned */
-  ART_ERR_WORKSPACE = -5, /* workspace NULL or too small for the *_host entry points */
+  ART_ERR_WORKSPACE = -5, /* workspace NULL, misaligned or too small where one is needed (the *_host entry point,
+                             split == ART_SPLIT_DYNAMIC) */
   ART_ERR_ARCH = -6,      /* current device is not compute capability 10.x */
   ART_ERR_CUDA = -7       /* a CUDA runtime call or the launch failed */
 };
