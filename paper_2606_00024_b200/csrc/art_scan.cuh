@@ -43,8 +43,8 @@ struct ScanCore {
 
   // Sums s[k][q] over the LPH lanes of each head.  Afterwards s[j][q], j < KH, holds the complete sums of
   // step owned_step(lane) + j.
-  template <int NB>
-  static __device__ __forceinline__ void reduce(float (&s)[NB][3], int lane) {
+  template <int NB, int Q>
+  static __device__ __forceinline__ void reduce(float (&s)[NB][Q], int lane) {
     constexpr int KH = kh<NB>();
     int cntk = NB;
 #pragma unroll
@@ -55,7 +55,7 @@ struct ScanCore {
 #pragma unroll
         for (int i = 0; i < half; ++i)
 #pragma unroll
-          for (int q = 0; q < 3; ++q) {
+          for (int q = 0; q < Q; ++q) {
             const float keep = up ? s[i + half][q] : s[i][q];
             const float send = up ? s[i][q] : s[i + half][q];
             s[i][q] = keep + __shfl_xor_sync(0xffffffffu, send, m);
@@ -65,7 +65,7 @@ struct ScanCore {
 #pragma unroll
         for (int i = 0; i < KH; ++i)
 #pragma unroll
-          for (int q = 0; q < 3; ++q) s[i][q] += __shfl_xor_sync(0xffffffffu, s[i][q], m);
+          for (int q = 0; q < Q; ++q) s[i][q] += __shfl_xor_sync(0xffffffffu, s[i][q], m);
       }
     }
   }
@@ -116,7 +116,7 @@ struct ScanCore {
       m_run = mn; l_run = l_new;
     }
     // ---- the recurrence x^(t) = x^(t-1) + r_t (P~V_t - l_t x^(t-1))   (l_t u^(t) = P~V_t)
-    float s[NB][3];
+    float sd[NB][1], sa[NB][2];                              // |dx|^2; (x_old . dx, |x_old|^2)
 #pragma unroll
     for (int k = 0; k < NB; ++k) {
       float pv[CPL];
@@ -128,10 +128,31 @@ struct ScanCore {
         sdd = fmaf(dlt, dlt, sdd); sad = fmaf(x[j], dlt, sad); saa = fmaf(x[j], x[j], saa);
         x[j] += dlt;
       }
-      s[k][0] = sdd; s[k][1] = sad; s[k][2] = saa;
+      sd[k][0] = sdd; sa[k][0] = sad; sa[k][1] = saa;
     }
-    reduce<NB>(s, lane);
     constexpr int KH = kh<NB>();
+    // A step can only be stable if every head passes the scale test (first half of Eq. 2).  Far from convergence
+    // none does, so |dx|^2 is summed over the lanes first and the two sums of the direction test only if needed:
+    // two thirds of the shuffles of a batch are saved in the common case, nothing is computed twice.
+    reduce<NB, 1>(sd, lane);
+    uint32_t pass = 0u;
+#pragma unroll
+    for (int j = 0; j < KH; ++j) {
+      const uint32_t v = __ballot_sync(0xffffffffu, sqrt_approx(sd[j][0]) < tau || (lane / LPH) >= g_real);
+#pragma unroll
+      for (int k = 0; k < NB; ++k) {
+        if (owner_slot<NB>(k) != j) continue;
+        uint32_t need = 0;
+#pragma unroll
+        for (int h = 0; h < G; ++h) need |= 1u << (h * LPH + owner_sub<NB>(k));
+        pass |= ((FULL || k < n) && (v & need) == need) ? (1u << k) : 0u;
+      }
+    }
+    if (pass == 0u) { cnt = (n > 0) ? 0 : cnt; return -1; }      // nobody stable: the counter is back at 0 (Eq. 3)
+    reduce<NB, 2>(sa, lane);
+    float s[KH][3];
+#pragma unroll
+    for (int j = 0; j < KH; ++j) { s[j][0] = sd[j][0]; s[j][1] = sa[j][0]; s[j][2] = sa[j][1]; }
     uint32_t votes[KH];
 #pragma unroll
     for (int j = 0; j < KH; ++j) votes[j] = __ballot_sync(0xffffffffu, stable_head(s[j], tau, phi) || (lane / LPH) >= g_real);
