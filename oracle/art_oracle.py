@@ -25,7 +25,11 @@ the G heads of a GQA group, one patience counter per group; R3 sink block first,
 then descending; R4 zero-norm => cos := 0 => d_direction = 1; R5 strict '<' for
 both tests, '>=' for the trigger; R6 probe on the normalised o^(t); R8 masked
 tokens have weight 0 and a block with no valid token still counts as a step;
-R9 stop_block = t* = number of blocks processed.
+R9 stop_block = t* = number of blocks processed; R15 (multi-token
+queries: speculative decode / the tail of a chunked prefill): the m query tokens of a
+sequence are its LAST m positions, query token i attends causally to the eligible
+tokens j <= L - m + i, the group walks its blocks ONCE for all m tokens and the
+criterion is the AND over all m * G (token, head) rows -- R2 with more rows.
 
 Parity pins: every function here is pinned by ``tests/test_oracle_*.py`` against
 closed forms, brute force, a library softmax, the paper's inequalities and a
@@ -172,10 +176,11 @@ def art_group(q: np.ndarray, K_blocks: np.ndarray, V_blocks: np.ndarray, valid: 
               sm_scale: float | None = None, trace: bool = False) -> GroupResult:
     """ART for one query group, Algorithm 1 step by step.
 
-    q        [G, d]      the G query heads sharing this KV head
+    q        [G, d]      the G query heads sharing this KV head (R15: the m * G (token, head) rows)
     K_blocks [T, 64, d]  keys of the eligible blocks IN TRAVERSAL ORDER
     V_blocks [T, 64, d]  values, same order
-    valid    [T, 64]     token-level eligibility (masked tokens get weight 0, R8)
+    valid    [T, 64]     token-level eligibility (masked tokens get weight 0, R8); or [G, T, 64], one mask per
+                         row (R15: the causal cut differs from query token to query token)
     """
     q = np.asarray(q, dtype=np.float64)
     G, d = q.shape
@@ -193,24 +198,24 @@ def art_group(q: np.ndarray, K_blocks: np.ndarray, V_blocks: np.ndarray, valid: 
     K = np.asarray(K_blocks, dtype=np.float64)
     V = np.asarray(V_blocks, dtype=np.float64)
     valid = np.asarray(valid, dtype=bool)
+    row_valid = np.broadcast_to(valid if valid.ndim == 3 else valid[None, :, :], (G, T, BLOCK_TOKENS))
+    anyrow = row_valid.any(axis=0)                              # [T, 64] eligible for at least one row
     # masked slots may hold garbage (even NaN) in a paged cache: never let them in
-    K = np.where(valid[:, :, None], K, 0.0)
-    V = np.where(valid[:, :, None], V, 0.0)
+    K = np.where(anyrow[:, :, None], K, 0.0)
+    V = np.where(anyrow[:, :, None], V, 0.0)
 
     # logits s_{h,t,j} = (q_h . k_{t,j}) / sqrt(d)   (Eq. 1)
     S = np.einsum("hd,tjd->htj", q, K) * scale
-    S = np.where(valid[None, :, :], S, -np.inf)
-    any_valid = bool(valid.any())
+    S = np.where(row_valid, S, -np.inf)
+    has = row_valid.reshape(G, -1).any(axis=1)                  # rows with at least one eligible token
     # first pass: global max over ALL eligible tokens (shift invariance of softmax)
-    M = S.reshape(G, -1).max(axis=1) if any_valid else np.zeros(G)
-    W = np.where(valid[None, :, :], np.exp(S - M[:, None, None]), 0.0)     # w_j = exp(s_j - M_h)
+    M = np.where(has, S.reshape(G, -1).max(axis=1), 0.0)
+    W = np.where(row_valid, np.exp(S - M[:, None, None]), 0.0)  # w_j = exp(s_j - M_h)
 
     # one-shot textbook softmax over E (Eq. 1), independent of the streaming below
-    if any_valid:
-        Wf = W.reshape(G, -1)
-        out_textbook = (Wf / Wf.sum(axis=1, keepdims=True)) @ V.reshape(-1, d)
-    else:
-        out_textbook = zeros.copy()
+    Wf = W.reshape(G, -1)
+    den = Wf.sum(axis=1, keepdims=True)
+    out_textbook = np.where(has[:, None], (Wf / np.where(den > 0, den, 1.0)) @ V.reshape(-1, d), 0.0)
 
     # ---- Algorithm 1 ----
     A = np.zeros(G)                   # A_0 = 0
@@ -299,21 +304,27 @@ def art_decode_attention_oracle(q, k_cache, v_cache, block_table, seq_lens, *,
                                 art: bool = True, groups=None, trace: bool = False):
     """Whole decode step: every (sequence b, KV head g) group, independently.
 
-    q [B, Hq, d]; k_cache / v_cache paged (layout above); block_table [B, max_blocks]
+    q [B, Hq, d], or [B, m, Hq, d] for m query tokens per sequence (R15: they are the last m positions,
+    whose K/V are already in the cache and counted in seq_lens; query token i sees tokens j <= L - m + i of
+    the policy's eligible set; rows of a group are ordered token-major, row = i * G + h);
+    k_cache / v_cache paged (layout above); block_table [B, max_blocks]
     logical block -> physical page; seq_lens [B]; eligible_blocks [B, Hkv, max_eligible]
     and eligible_counts [B, Hkv] for POLICY_LIST.  GQA: query head h belongs to KV head
     h // G (paper silent; standard).  art=False disables termination (ART-off): the
     result is o^(T) and stop_block = T.
 
-    Returns (out [B, Hq, d] float64, stop_block [B, Hkv] int64, results dict keyed (b, g)).
+    Returns (out [B, Hq, d] (or [B, m, Hq, d]) float64, stop_block [B, Hkv] int64, results dict keyed (b, g)).
     `groups` optionally restricts the work to a list of (b, g) pairs; other rows stay 0.
     """
     q = np.asarray(q, dtype=np.float64)
-    B, Hq, d = q.shape
+    multi = q.ndim == 4
+    if not multi:
+        q = q[:, None]
+    B, m, Hq, d = q.shape
     Hkv = int(num_kv_heads)
     assert Hq % Hkv == 0
     G = Hq // Hkv
-    out = np.zeros((B, Hq, d))
+    out = np.zeros((B, m, Hq, d))
     stop = np.zeros((B, Hkv), dtype=np.int64)
     results = {}
     todo = groups if groups is not None else [(b, g) for b in range(B) for g in range(Hkv)]
@@ -330,14 +341,18 @@ def art_decode_attention_oracle(q, k_cache, v_cache, block_table, seq_lens, *,
         safe_blocks = [blk if valid[i].any() else 0 for i, blk in enumerate(blocks)]
         Kb = gather_group_blocks(k_cache, layout, block_table[b], g, safe_blocks)
         Vb = gather_group_blocks(v_cache, layout, block_table[b], g, safe_blocks)
-        r = art_group(q[b, g * G:(g + 1) * G], Kb, Vb, valid,
+        if m > 1 and len(blocks):                               # R15: causal cut per query token
+            pos = np.asarray(blocks)[:, None] * BLOCK_TOKENS + np.arange(BLOCK_TOKENS)[None, :]     # [T, 64]
+            cut = np.stack([pos < L - (m - 1 - i) for i in range(m)])                               # [m, T, 64]
+            valid = np.repeat(valid[None] & cut, G, axis=0)     # row i * G + h
+        r = art_group(q[b, :, g * G:(g + 1) * G].reshape(m * G, d), Kb, Vb, valid,
                       tau=tau if art else 0.0, phi=phi if art else 0.0,
                       patience=patience if art else PATIENCE_INF,
                       probe_dim=probe_dim, sm_scale=sm_scale, trace=trace)
-        out[b, g * G:(g + 1) * G] = r.out_on
+        out[b, :, g * G:(g + 1) * G] = r.out_on.reshape(m, G, d)
         stop[b, g] = r.stop_block
         results[(b, g)] = r
-    return out, stop, results
+    return (out if multi else out[:, 0]), stop, results
 
 
 # --------------------------------------------------------------------------- base-policy block list
