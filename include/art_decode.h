@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define ART_VERSION 100          /* 0.1.0 */
+#define ART_VERSION 110          /* 0.1.1: art_desc_t.q_len */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
 #define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent grid, steps claimed at run time (BF16 only) */
 #define ART_PATIENCE_INF 2147483647 /* "p = infinity": detector runs, never fires (App. E) */
@@ -44,9 +44,10 @@ extern "C" {
 enum {
   ART_OK = 0,
   ART_ERR_NULL = -1,      /* a required pointer is NULL */
-  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G = Hq / Hkv > 8, unsupported head_dim, block_tokens != 64,
-                             negative sizes, policy/list mismatch, bad thresholds */
-  ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128) */
+  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G = Hq / Hkv > 8, q_len * G > 8, q_len > 1 with ART_SPLIT_DYNAMIC,
+                             unsupported head_dim, block_tokens != 64, negative sizes, policy/list mismatch,
+                             bad thresholds */
+  ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128; q_len > 1: BF16) */
   ART_ERR_ALIGN = -4,     /* q / k_cache / v_cache not 16-byte aligned */
   ART_ERR_WORKSPACE = -5, /* workspace NULL, misaligned or too small where one is needed (the *_host entry point,
                              split == ART_SPLIT_DYNAMIC) */
@@ -83,6 +84,13 @@ typedef struct art_desc {
                                   ART_SPLIT_DYNAMIC: no fixed binding, a persistent grid whose CTAs claim steps
                                   of whichever group has work left (needs `workspace`).  Any value gives the
                                   same stop_block as the sequential algorithm. */
+  int32_t q_len;               /* m: query tokens per sequence (speculative decode, the tail of a chunked
+                                  prefill); 0 or 1 = plain decode.  The m tokens are the LAST m positions of the
+                                  sequence (their K/V are in the cache and counted in seq_lens); query token i attends
+                                  to the eligible tokens j <= L - m + i; the group walks its blocks once and the
+                                  criterion is the AND over all m * G (token, head) rows (reading R15).
+                                  m > 1 needs m * G <= 8, BF16 and a cluster schedule (split >= 0); q and out are
+                                  then [B, m, Hq, d]. */
   const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
   int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
                                   (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */
@@ -100,14 +108,14 @@ typedef struct art_thresholds {
  * ART-on decode attention.  Enqueues on `cuda_stream` (a cudaStream_t, NULL = default
  * stream) and returns; results are valid once the stream has been synchronised.
  *
- *   q               DEVICE [B, Hq, d]            dtype elements, 16-B aligned
+ *   q               DEVICE [B, Hq, d]            dtype elements, 16-B aligned ([B, m, Hq, d] when q_len = m > 1)
  *   k_cache,v_cache DEVICE paged caches (kv_layout), dtype elements, 16-B aligned
  *   block_table     DEVICE int32 [B, max_blocks_per_seq]  logical block -> physical page
  *   eligible_blocks DEVICE int32 [B, Hkv, max_eligible]   LOGICAL block ids, distinct, walked in the
  *                   order given; NULL unless policy == LIST
  *   seq_lens        DEVICE int32 [B]; tokens >= seq_lens[b] of the last block are masked
  *   thresholds      HOST
- *   out             DEVICE float32 [B, Hq, d]    o^(t*) (Alg. 1 l.18)
+ *   out             DEVICE float32 [B, Hq, d]    o^(t*) (Alg. 1 l.18) ([B, m, Hq, d] when q_len = m > 1)
  *   stop_block      DEVICE int32 [B, Hkv]        t* = number of blocks processed, in [0, T];
  *                                                T if the criterion never fired
  *   workspace       DEVICE scratch, 256-B aligned, >= art_workspace_bytes(desc); only read and written when
@@ -164,7 +172,7 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
  *                             ties -> lower block index first (reading R10); eligible_counts[b, g] = their number
  * The outputs are what art_decode_attention takes with policy == LIST.  Uses desc->{batch, num_q_heads,
  * num_kv_heads, head_dim, block_tokens, dtype, kv_layout, max_blocks_per_seq (<= 4096), max_eligible (row stride
- * of eligible_blocks, >= top_k)}.  q, k_cache, block_table, seq_lens as above; block_scores DEVICE float32
+ * of eligible_blocks, >= top_k)}; q_len must be 0 or 1.  q, k_cache, block_table, seq_lens as above; block_scores DEVICE float32
  * [B, Hkv, max_blocks_per_seq]; eligible_blocks DEVICE int32 [B, Hkv, max_eligible]; eligible_counts DEVICE
  * int32 [B, Hkv].  Enqueues two kernels on cuda_stream and returns.  Entries beyond the count are not written.
  */

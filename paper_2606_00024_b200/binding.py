@@ -28,7 +28,7 @@ class ArtDesc(C.Structure):
         ("head_dim", C.c_int32), ("block_tokens", C.c_int32), ("dtype", C.c_int32),
         ("kv_layout", C.c_int32), ("policy", C.c_int32), ("max_blocks_per_seq", C.c_int32),
         ("sink_tokens", C.c_int32), ("window_tokens", C.c_int32), ("max_eligible", C.c_int32),
-        ("sm_scale", C.c_float), ("split", C.c_int32),
+        ("sm_scale", C.c_float), ("split", C.c_int32), ("q_len", C.c_int32),
         ("eligible_counts", C.c_void_p), ("blocks_loaded", C.c_void_p),
     ]
 
@@ -179,7 +179,8 @@ def art_topk_blocks(desc, q, k_cache, block_table, seq_lens, top_k, block_scores
 # ------------------------------------------------------------------ convenience (argument marshalling only)
 
 def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None, sm_scale: float = 0.0) -> ArtDesc:
-    """Fill an art_desc_t from a workload-like object (fields as in workloads.generators.Workload)."""
+    """Fill an art_desc_t from a workload-like object (fields as in workloads.generators.Workload).
+    A 4-D w.q is [B, m, Hq, d]: m query tokens per sequence (art_desc_t.q_len)."""
     ec = eligible_counts if eligible_counts is not None else w.eligible_counts
     return ArtDesc(
         batch=w.batch, num_q_heads=w.num_q_heads, num_kv_heads=w.num_kv_heads, head_dim=w.head_dim,
@@ -187,7 +188,7 @@ def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None, sm
         kv_layout=w.layout, policy=w.policy, max_blocks_per_seq=int(w.block_table.shape[1]),
         sink_tokens=w.sink_tokens, window_tokens=w.window_tokens,
         max_eligible=0 if w.eligible_blocks is None else int(w.eligible_blocks.shape[2]),
-        sm_scale=sm_scale, split=split,
+        sm_scale=sm_scale, split=split, q_len=int(w.q.shape[1]) if w.q.dim() == 4 else 0,
         eligible_counts=None if ec is None else ec.data_ptr(),
         blocks_loaded=None if blocks_loaded is None else blocks_loaded.data_ptr())
 
@@ -195,9 +196,9 @@ def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None, sm
 def run_workload(w, *, art: bool = True, split: int = 0, tau=None, phi=None, patience=None, probe_dim=None,
                  want_loaded: bool = False, stream=None, sm_scale: float = 0.0):
     """Allocate outputs and run one decode step on a CUDA-resident workload.
-    Returns (out [B,Hq,d] fp32, stop_block [B,Hkv] int32, blocks_loaded or None)."""
+    Returns (out [B,Hq,d] (or [B,m,Hq,d]) fp32, stop_block [B,Hkv] int32, blocks_loaded or None)."""
     dev = w.q.device
-    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32, device=dev)
+    out = torch.empty(tuple(w.q.shape), dtype=torch.float32, device=dev)
     stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev)
     loaded = torch.zeros((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev) if want_loaded else None
     desc = make_desc(w, split=split, blocks_loaded=loaded, sm_scale=sm_scale)

@@ -32,7 +32,9 @@ struct Params {
   int32_t* stop_block;
   int32_t* blocks_loaded;
   int32_t batch, Hq, Hkv;
-  int32_t Gr;                                        // real heads per group (Hq / Hkv); kernels are built for the next power of two
+  int32_t Gr;                                        // real rows per group (q_len * Hq / Hkv); kernels are built for the next power of two
+  int32_t Gh, qlen;                                  // heads per query token of a group (Hq / Hkv), query tokens m (R15); row = i * Gh + h
+  uint32_t cuts;                                     // 4 bits per row: m - 1 - i, the most recent tokens row i may not see; 0 when m == 1
   int32_t max_blocks, max_elig;
   int32_t policy, layout, sink, window;
   int64_t page_stride, head_stride, token_stride;   // bytes

@@ -22,6 +22,9 @@ namespace art {
 
 // kernels are instantiated for 1, 2, 4, 8 heads per group; other group sizes run the next one up with padding heads
 static inline int padded_group(int g) { return g <= 1 ? 1 : (g <= 2 ? 2 : (g <= 4 ? 4 : 8)); }
+static inline int qlen_of(const art_desc_t* d) { return d->q_len > 1 ? d->q_len : 1; }
+// rows a group carries through its walk: one per (query token, head) pair (reading R15)
+static inline int rows_of(const art_desc_t* d) { return (d->num_q_heads / d->num_kv_heads) * qlen_of(d); }
 
 struct LaunchPlan { int C, stages, mslots; uint32_t smem; };
 
@@ -171,6 +174,12 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
   if (d->num_q_heads % d->num_kv_heads != 0) return ART_ERR_SHAPE;
   const int G = d->num_q_heads / d->num_kv_heads;
   if (G > 8) return ART_ERR_SHAPE;
+  if (d->q_len < 0 || d->q_len > 8 || G * qlen_of(d) > 8) return ART_ERR_SHAPE;
+  if (d->q_len > 1) {                                   // built for the bf16 cluster kernel only
+    if (d->dtype == ART_DTYPE_F32) return ART_ERR_DTYPE;
+    if (d->split == ART_SPLIT_DYNAMIC) return ART_ERR_SHAPE;
+    if (d->max_blocks_per_seq >= (1 << 24) || d->max_eligible >= (1 << 24)) return ART_ERR_SHAPE;
+  }
   if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
   if (d->dtype != ART_DTYPE_F32 && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (d->head_dim != 64 && d->head_dim != 128) return ART_ERR_SHAPE;
@@ -274,7 +283,7 @@ static int cluster_capacity(const art_desc_t* d, int G, int mode, int C, uint32_
 // group streams from the first cycle; never more CTAs than a group could have blocks.  The tensor-core
 // kernel takes any C (steps are dealt round-robin); the CUDA-core kernel's mailbox wants a power of two.
 static int choose_split(const art_desc_t* d, int mode, int* C_out) {
-  const int G = padded_group(d->num_q_heads / d->num_kv_heads);
+  const int G = padded_group(rows_of(d));
   const int groups = d->batch * d->num_kv_heads;
   const bool art = mode != 0;
   const int PW = mode == 2 ? d->head_dim : 32;
@@ -342,7 +351,7 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
                cudaStream_t stream) {
   const int groups = d->batch * d->num_kv_heads;
   if (groups == 0) return ART_OK;
-  const int G = padded_group(d->num_q_heads / d->num_kv_heads);
+  const int G = padded_group(rows_of(d));
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
@@ -356,7 +365,9 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   p.q = q; p.k = static_cast<const uint8_t*>(k); p.v = static_cast<const uint8_t*>(v);
   p.block_table = bt; p.elig = elig; p.elig_counts = elig_counts; p.seq_lens = sl;
   p.out = out; p.stop_block = stop; p.blocks_loaded = blocks_loaded;
-  p.batch = d->batch; p.Hq = d->num_q_heads; p.Hkv = d->num_kv_heads; p.Gr = d->num_q_heads / d->num_kv_heads;
+  p.batch = d->batch; p.Hq = d->num_q_heads; p.Hkv = d->num_kv_heads;
+  p.Gh = d->num_q_heads / d->num_kv_heads; p.qlen = qlen_of(d); p.Gr = p.Gh * p.qlen;
+  for (int r = 0; r < p.Gr; ++r) p.cuts |= static_cast<uint32_t>(p.qlen - 1 - r / p.Gh) << (4 * r);
   p.max_blocks = d->max_blocks_per_seq; p.max_elig = d->max_eligible;
   p.policy = d->policy; p.layout = d->kv_layout; p.sink = d->sink_tokens; p.window = d->window_tokens;
   const int64_t row = kRowBytes;
@@ -399,6 +410,9 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
     if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
       return ART_ERR_CUDA;
     e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
+      if (p.qlen > 1)
+        return static_cast<int>(launch_cluster(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value, true>,
+                                               tc::kThreads, groups, C, pl.smem, stream, p, tmK, tmV));
       return static_cast<int>(launch_cluster(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value>,
                                              tc::kThreads, groups, C, pl.smem, stream, p, tmK, tmV));
     }));
@@ -470,7 +484,7 @@ static HostLayout host_layout(const art_desc_t* d) {
   auto up = [](size_t x) { return (x + 255) & ~static_cast<size_t>(255); };
   HostLayout h; size_t off = 0;
   const size_t esz = d->dtype == ART_DTYPE_F32 ? 4 : 2;
-  const size_t B = d->batch, Hq = d->num_q_heads, Hkv = d->num_kv_heads, D = d->head_dim;
+  const size_t B = d->batch, Hq = static_cast<size_t>(d->num_q_heads) * art::qlen_of(d), Hkv = d->num_kv_heads, D = d->head_dim;   // Hq: query rows per sequence
   h.q = off; off = up(off + B * Hq * D * esz);
   h.bt = off; off = up(off + B * static_cast<size_t>(d->max_blocks_per_seq) * 4);
   h.sl = off; off = up(off + B * 4);
@@ -503,7 +517,7 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   uint8_t* ws = static_cast<uint8_t*>(workspace);
   const size_t esz = desc->dtype == ART_DTYPE_F32 ? 4 : 2;
-  const size_t B = desc->batch, Hq = desc->num_q_heads, Hkv = desc->num_kv_heads, D = desc->head_dim;
+  const size_t B = desc->batch, Hq = static_cast<size_t>(desc->num_q_heads) * art::qlen_of(desc), Hkv = desc->num_kv_heads, D = desc->head_dim;
   if (B == 0) return ART_OK;
   bool ok = true;
   {
@@ -572,7 +586,7 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
                     int32_t* eligible_counts, void* cuda_stream) {
   if (!d || !q || !k_cache || !block_table || !seq_lens || !block_scores || !eligible_blocks || !eligible_counts) return ART_ERR_NULL;
   if (d->batch < 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads) return ART_ERR_SHAPE;
-  if (d->num_q_heads / d->num_kv_heads > 8) return ART_ERR_SHAPE;
+  if (d->num_q_heads / d->num_kv_heads > 8 || d->q_len > 1) return ART_ERR_SHAPE;    // scores are defined for one query token
   const int G = art::padded_group(d->num_q_heads / d->num_kv_heads);
   if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
   if (!((d->dtype == ART_DTYPE_F32 && d->head_dim == 64) || (d->dtype == ART_DTYPE_BF16 && d->head_dim == 128))) return ART_ERR_DTYPE;
@@ -617,7 +631,8 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
 int art_query_split(const art_desc_t* desc, int art_on) {
   if (!desc) return ART_ERR_NULL;
   if (desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->num_q_heads % desc->num_kv_heads) return ART_ERR_SHAPE;
-  if (desc->num_q_heads / desc->num_kv_heads > 8) return ART_ERR_SHAPE;
+  if (desc->num_q_heads / desc->num_kv_heads > 8 || desc->q_len < 0 || art::rows_of(desc) > 8) return ART_ERR_SHAPE;
+  if (desc->q_len > 1 && desc->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;

@@ -116,6 +116,16 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
 }
 constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8, kNext = 12, kNTotal = 16;
 
+// An entry of the item ring: the step number in the low 24 bits and, for multi-token queries (R15), the causal
+// code of the step's block above them: e = L - 64 * blk (tokens of the sequence from the start of this block on)
+// when the causal cut of some row can reach into the block (1 <= e <= 70: a row loses at most 7 tokens), else 0.
+// Row r then sees token `tok` of the block iff tok + cut_r < e.
+constexpr int kItemShift = 24, kItemStep = (1 << kItemShift) - 1;
+__device__ __forceinline__ int causal_code(const Params& p, int L, int blk) {
+  const int e = L - blk * kBlockTokens;
+  return (e >= 1 && e < kBlockTokens + 7) ? e : 0;
+}
+
 // ----------------------------------------------------------------------------- tcgen05 / TMA wrappers
 
 __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* tm, int c0, int c1, int c2, uint32_t bar) {
@@ -230,7 +240,9 @@ template <int G> __device__ __forceinline__ int head_of_lane32(int lane) {
 // ----------------------------------------------------------------------------- the kernel
 
 // MODE 0: ART off.  MODE 1: ART on, probe = 32 coordinates k*(d/32).  MODE 2: ART on, probe = all d.
-template <int G, int MODE>
+// MT: multi-token queries (reading R15) -- rows are (query token, head) pairs and the most recent tokens are cut
+// row by row; compiled apart so that plain decode carries none of it.
+template <int G, int MODE, bool MT = false>
 __global__ void __launch_bounds__(kThreads, (MODE == 2) ? 1 : 2)
 art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
   constexpr bool ART = MODE != 0;
@@ -264,6 +276,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   const int n_lim = p.dyn ? 0x7fffffff : n_c;                 // items this CTA will process, if known up front
   constexpr int kItemT = item_ring(G, MODE == 1);
   int* item_t = reinterpret_cast<int*>(smem + sm.items);      // step number of item i (i mod kItemT)
+  auto item_step = [](int v) { return MT ? (v & kItemStep) : v; };
   const uint32_t a_ntotal = sbase + sm.misc + kNTotal;
 
 #ifdef ART_TRACE
@@ -288,10 +301,11 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   }
   if (warp == kWarpMmaPV) tmem_alloc(a_tmem, kTmemCols);
   {
-    const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD;
+    // row = i * Gh + h: head h of the group for query token i (R15; one token: row == head)
+    const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.q) + (static_cast<int64_t>(b) * p.qlen * p.Hq + g * p.Gh) * kD;
     for (int idx = tid; idx < 8 * kD; idx += kThreads) {       // rows >= G: zeros (rows 8-15 alias, see kQLbo)
       const int row = idx / kD, dc = idx % kD;
-      const __nv_bfloat16 v = (row < p.Gr) ? qp[row * kD + dc] : __float2bfloat16_rn(0.f);
+      const __nv_bfloat16 v = (row < p.Gr) ? qp[((row / p.Gh) * p.Hq + row % p.Gh) * kD + dc] : __float2bfloat16_rn(0.f);
       *reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + (dc >> 3) * kQLbo + row * 16 + (dc & 7) * 2) = v;
     }
     if (tid < 64) reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + 16 * kQLbo)[tid] = __float2bfloat16_rn(0.f);
@@ -343,12 +357,13 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         return static_cast<int>(r) + 1;
       };
       // resolve a claimed step: validity, token mask, page (the table lookup is left in flight)
-      auto resolve = [&](int t, bool& valid, unsigned long long& mask, int& page) {
+      auto resolve = [&](int t, bool& valid, unsigned long long& mask, int& page, int& ec) {
         valid = t <= Tn && !beyond_stop(t);                     // exhausted, or beyond t* (A7: stop prefetching)
-        mask = 0ull; page = 0;
+        mask = 0ull; page = 0; ec = 0;
         if (valid) {
           const int blk = trav_block(tr, t);
           mask = block_mask(p, L, blk);
+          if constexpr (MT) ec = causal_code(p, L, blk);
           if (mask) page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
         }
       };
@@ -356,20 +371,20 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       int tB = 0;
       if (lane == 0) tB = claim();
       int tA = __shfl_sync(0xffffffffu, tB, 0);
-      bool validA; unsigned long long maskA; int pageA;
-      resolve(tA, validA, maskA, pageA);
+      bool validA; unsigned long long maskA; int pageA, ecA;
+      resolve(tA, validA, maskA, pageA, ecA);
       if (lane == 0) tB = claim();
       while (validA) {
         const int tN = __shfl_sync(0xffffffffu, tB, 0);
-        bool validB; unsigned long long maskB; int pageB;
-        resolve(tN, validB, maskB, pageB);
+        bool validB; unsigned long long maskB; int pageB, ecB;
+        resolve(tN, validB, maskB, pageB, ecB);
         if (validB && lane == 0) tB = claim();
         if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                  // slot released?
         if (lane == 0) {
           TC_TRACE(trc, 1, group, tA);
           const uint32_t fb = bar(sm.full0 + stage);
           const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
-          item_t[it % kItemT] = tA;
+          item_t[it % kItemT] = tA | (ecA << kItemShift);
           sinfo[stage] = maskA;
           if (maskA == 0ull) {
             mbar_arrive(fb);                                   // nothing to load: an all-masked step
@@ -387,7 +402,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (maskA != 0ull) ++loaded;
         ++it;
         if (++stage == S) { stage = 0; ph ^= 1u; }
-        tA = tN; validA = validB; maskA = maskB; pageA = pageB;
+        tA = tN; validA = validB; maskA = maskB; pageA = pageB; ecA = ecB;
       }
       it_issued = it;
     } else {
@@ -396,10 +411,11 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       bool stop = false;
       for (int i0 = 0; i0 < n_c && !stop; i0 += 32) {
         const int i = i0 + lane;
-        unsigned long long mask = 0ull; int c1 = 0, c2 = 0;
+        unsigned long long mask = 0ull; int c1 = 0, c2 = 0, ec = 0;
         if (i < n_c) {
           const int blk = trav_block(tr, step_of(i));
           mask = block_mask(p, L, blk);
+          if constexpr (MT) ec = causal_code(p, L, blk);
           if (mask) {
             const int page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
             if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = page * p.Hkv + g; }     // [page*Hkv + head][token][d]
@@ -411,13 +427,15 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
           const int it = i0 + kk, t = step_of(it);
           const unsigned long long mask_k = __shfl_sync(0xffffffffu, mask, kk);
           const int c1_k = __shfl_sync(0xffffffffu, c1, kk), c2_k = __shfl_sync(0xffffffffu, c2, kk);
+          int ec_k = 0;
+          if constexpr (MT) ec_k = __shfl_sync(0xffffffffu, ec, kk);
           if (beyond_stop(t)) { stop = true; break; }          // A7: stop issuing prefetch once fired
           if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                // slot released?
           if (lane == 0) {
             TC_TRACE(trc, 1, group, t);
             const uint32_t fb = bar(sm.full0 + stage);
             const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
-            item_t[it % kItemT] = t;
+            item_t[it % kItemT] = t | (ec_k << kItemShift);
             sinfo[stage] = mask_k;
             if (mask_k == 0ull) {
               mbar_arrive(fb);                                 // nothing to load: an all-masked step
@@ -518,11 +536,23 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       const unsigned long long vmask = sinfo[st];             // written before the loads the S MMA waited for
       const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
       float mb[G];
+      int ec = 0;
+      if constexpr (MT) ec = item_t[i % kItemT] >> kItemShift;
+      if (MT && ec != 0) {                                    // R15: the most recent tokens are cut row by row
 #pragma unroll
-      for (int h = 0; h < G; ++h) {
-        s0[h] = v0 ? s0[h] * p.scale_log2 : kNegInf;          // masked tokens: weight 0 (R8); their K may be NaN
-        s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
-        mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
+        for (int h = 0; h < G; ++h) {
+          const int lim = ec - static_cast<int>((p.cuts >> (4 * h)) & 15u);
+          s0[h] = (v0 && lane < lim) ? s0[h] * p.scale_log2 : kNegInf;
+          s1[h] = (v1 && lane + 32 < lim) ? s1[h] * p.scale_log2 : kNegInf;
+          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
+        }
+      } else {
+#pragma unroll
+        for (int h = 0; h < G; ++h) {
+          s0[h] = v0 ? s0[h] * p.scale_log2 : kNegInf;        // masked tokens: weight 0 (R8); their K may be NaN
+          s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
+          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
+        }
       }
       uint8_t* pb0 = smem + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;   // token `lane`, row 0, hi
       float ls[G];
@@ -592,7 +622,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         }
       }
       release_pv(i);
-      if (tid == 0) TC_TRACE(trf, 5, i, item_t[i % kItemT]);
+      if (tid == 0) TC_TRACE(trf, 5, i, item_step(item_t[i % kItemT]));
     };
     if constexpr (!ART) {
       for (int i = 0; i < n_lim; ++i) {
@@ -609,7 +639,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         // ---- merge the oldest unfolded block once the decision for the steps before it is known; one that
         //      lies beyond t* is dropped (its tensor-memory slot is released, nothing is merged)
         if (fld < pub) {
-          const int tf = item_t[fld % kItemT];
+          const int tf = item_step(item_t[fld % kItemT]);
           if (c < 0 && tf > -c) { release_pv(fld); ++fld; continue; }
           if (c < 0 || c >= tf - 1) { fold(fld); ++fld; continue; }
         }
@@ -619,7 +649,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
           const uint32_t par = (pub / NP) & 1;
           if (!pub_ready) pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
           if (pub_ready && c < 0) { ++pub; pub_ready = false; continue; }   // fired: an unpublished step lies beyond t*
-          const int t = pub_ready ? item_t[pub % kItemT] : 0;
+          const int t = pub_ready ? item_step(item_t[pub % kItemT]) : 0;
           if (pub_ready && c >= t - M) {                      // mailbox slot free: step t - M has been scanned
             const int slot_i = (t - 1) & (M - 1);
             tc_fence_after();
@@ -721,7 +751,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         a = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta[o]), c)), a);
         l = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta_l[h]), c)), l);
       }
-      if (h < p.Gr) p.out[(static_cast<int64_t>(b) * p.Hq + g * p.Gr) * kD + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
+      if (h < p.Gr)                                             // Alg. 1 l.18; row h = query token h / Gh, head h % Gh
+        p.out[((static_cast<int64_t>(b) * p.qlen + h / p.Gh) * p.Hq + g * p.Gh + h % p.Gh) * kD + (o - h * kD)] = (l > 0.f) ? a / l : 0.f;
     }
     if (tid == 0) {
       if (!ART) p.stop_block[group] = Tn;

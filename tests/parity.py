@@ -49,14 +49,16 @@ def compare(w_host, out_gpu: torch.Tensor, stop_gpu: torch.Tensor, *, art: bool,
                 mism_f += 1
                 continue                       # a legitimately different stop: outputs not comparable
             mism_nf += 1
+        d = o_ref.shape[-1]
         for h in range(g * G, (g + 1) * G):
-            ref = o_ref[b, h]
-            scale = np.abs(ref).max()
-            err = np.abs(out[b, h] - ref).max()
-            if not np.isfinite(err):
-                max_rel = float("inf")
-            elif scale > 0:
-                max_rel = max(max_rel, err / scale)
-            elif err > 0:
-                max_rel = float("inf")
+            # one row per query token (q [B, m, Hq, d], reading R15), else the head's single row
+            for ref, got in zip(o_ref[b, ..., h, :].reshape(-1, d), out[b, ..., h, :].reshape(-1, d)):
+                scale = np.abs(ref).max()
+                err = np.abs(got - ref).max()
+                if not np.isfinite(err):
+                    max_rel = float("inf")
+                elif scale > 0:
+                    max_rel = max(max_rel, err / scale)
+                elif err > 0:
+                    max_rel = float("inf")
     return ParityReport(len(res), mism_nf, mism_f, frag, max_rel, fired, float(np.mean(fr)) if fr else 0.0)

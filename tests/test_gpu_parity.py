@@ -356,3 +356,81 @@ def test_full_size_sampled(index, sub, variant):
             assert np.array_equal(s_g.cpu().numpy(), s_ref)
     del w
     torch.cuda.empty_cache()
+
+
+# ------------------------------------------------------------------ multi-token queries (reading R15)
+
+def multi_workload(m, G, *, Hkv=2, lens=(1500, 777), seed=5, decay=None, policy=gen.POLICY_DENSE, layout=gen.LAYOUT_HND, **kw):
+    w = gen.make_workload("multi", seed=seed, batch=len(lens), num_q_heads=G * Hkv, num_kv_heads=Hkv, head_dim=128,
+                          seq_lens=list(lens), planted_frac=0.01, sink_plant=4, recency_decay=decay, policy=policy,
+                          layout=layout, **kw)
+    return gen.with_query_tokens(w, m, seed=seed + 100 * m)
+
+
+@pytest.mark.parametrize("m,G", [(2, 4), (2, 1), (3, 2), (4, 2), (8, 1), (5, 1), (2, 3)])
+@pytest.mark.parametrize("split", [0, 1, 3])
+def test_multi_token_off_and_literal(m, G, split):
+    """Every (token, head) row against the oracle: causal cut per query token, ragged tails (777 = 12 * 64 + 9)."""
+    w = multi_workload(m, G)
+    check(w, art_on=False, split=split)
+    check(w, split=split)                       # paper-default thresholds: the detector runs, never fires
+
+
+@pytest.mark.parametrize("m,G", [(2, 4), (4, 2), (8, 1), (3, 1)])
+@pytest.mark.parametrize("split", [1, 2, 4, 8])
+def test_multi_token_firing(m, G, split):
+    """One decision per group, AND over all m * G rows: stop blocks bit-exact against the oracle."""
+    w = multi_workload(m, G, decay=(0.2, 1.0), lens=(4096, 3000))
+    _, stop, _, rep = check(w, split=split, tau=1e-3, expect_fired=True)
+    assert rep.mean_stop_frac < 0.9
+
+
+@pytest.mark.parametrize("L", [1, 2, 3, 7, 63, 64, 65, 66, 70, 71, 127, 128, 129, 135])
+def test_multi_token_block_boundaries(L):
+    """The causal cut straddling a block boundary, rows whose first step is empty, L < m (zero rows)."""
+    for m, G in [(4, 2), (8, 1)]:
+        w = multi_workload(m, G, Hkv=1, lens=(L, max(1, L - 1)), seed=L)
+        out, _, _, _ = check(w, art_on=False)
+        check(w, tau=1e9, phi=2.5, patience=1)  # everything passes: stops at the first step all rows have a token
+        if L < m:
+            assert torch.equal(out[0, :m - L].cpu(), torch.zeros_like(out[0, :m - L].cpu()))
+
+
+@pytest.mark.parametrize("policy", ["sink_window", "list"])
+def test_multi_token_sparse_policies(policy):
+    if policy == "sink_window":
+        w = multi_workload(2, 4, policy=gen.POLICY_SINK_WINDOW, sink_tokens=70, window_tokens=300, lens=(1500, 777))
+    else:
+        w = multi_workload(2, 4, policy=gen.POLICY_LIST, topk_blocks=8, lens=(1500, 777))
+    check(w, art_on=False)
+    check(w, tau=1e-3)
+    w2 = multi_workload(2, 4, layout=gen.LAYOUT_NHD)
+    check(w2, art_on=False)
+
+
+def test_multi_token_one_token_is_the_plain_call():
+    """q_len = 1 through the 4-D path equals the 3-D call bit for bit (ART-off: statically dealt steps)."""
+    from dataclasses import replace
+    w = multi_workload(2, 4)
+    w1 = replace(w, q=w.q[:, 1].contiguous())
+    w1m = replace(w, q=w.q[:, 1:2].contiguous())
+    a = art()
+    o1, s1, _ = a.run_workload(w1.to("cuda"), art=False)
+    o2, s2, _ = a.run_workload(w1m.to("cuda"), art=False)
+    assert torch.equal(o1, o2[:, 0]) and torch.equal(s1, s2)
+
+
+def test_multi_token_host_entry():
+    """The host entry point stages q [B, m, Hq, d] and returns out [B, m, Hq, d]."""
+    a = art()
+    w = multi_workload(2, 4, decay=(0.2, 1.0), lens=(4096, 3000))
+    wc = w.to("cuda")
+    desc = a.make_desc(wc)
+    ws = torch.empty(max(a.art_workspace_bytes(desc), 256), dtype=torch.uint8, device="cuda")
+    th = a.ArtThresholds(tau=1e-3, phi=w.phi, patience=w.patience, probe_dim=w.probe_dim)
+    out_h = torch.empty(tuple(w.q.shape), dtype=torch.float32).pin_memory()
+    stop_h = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32).pin_memory()
+    a.art_decode_attention_host(desc, w.q.pin_memory(), wc.k_cache, wc.v_cache, w.block_table.pin_memory(), None,
+                                w.seq_lens.pin_memory(), th, out_h, stop_h, ws)
+    rep = compare(w, out_h, stop_h, art=True, oracle_over=dict(tau=f32(1e-3)))
+    assert rep.ok(OUT_TOL[w.dtype]) and rep.fired_groups > 0, rep

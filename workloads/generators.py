@@ -303,3 +303,18 @@ def config(index: int, *, device="cpu", variant: str = "", scale: float = 1.0, b
         raise ValueError("config index 0..4")
     kw.update(over)
     return make_workload(name, device=device, layout=layout, **kw)
+
+
+def with_query_tokens(w: Workload, m: int, *, seed: int, jitter: float = 0.5) -> Workload:
+    """Multi-token variant of a decode step (speculative decode / the tail of a chunked prefill):
+    q becomes [B, m, Hq, d].  The LAST query token is the workload's own; the m - 1 before it are that query plus
+    N(0, jitter^2) noise per coordinate (scaled by the query's rms), as neighbouring positions of one sequence
+    ask similar questions.  The cache is untouched: its last m positions are taken to be the query tokens'."""
+    from dataclasses import replace
+    gen = _gen(seed, w.q.device)
+    q32 = w.q.to(torch.float32)
+    rms = q32.pow(2).mean(dim=-1, keepdim=True).sqrt()
+    toks = [q32 + jitter * rms * torch.randn(q32.shape, generator=gen, device=w.q.device, dtype=torch.float32)
+            for _ in range(m - 1)] + [q32]
+    return replace(w, q=torch.stack(toks, dim=1).to(w.dtype).contiguous())
+
