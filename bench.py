@@ -158,7 +158,7 @@ def make_runner(art, w, *, art_on: bool, split: int = 0, **th):
     """Pre-marshalled call (descriptors and outputs allocated once); returns (fn, out, stop, loaded)."""
     import torch
     dev = w.q.device
-    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32, device=dev)
+    out = torch.empty(tuple(w.q.shape), dtype=torch.float32, device=dev)        # [B, Hq, d], or [B, m, Hq, d]
     stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev)
     loaded = torch.zeros((w.batch, w.num_kv_heads), dtype=torch.int32, device=dev)
     desc = art.make_desc(w, split=split, blocks_loaded=loaded)
@@ -178,7 +178,7 @@ def make_host_runner(art, w, *, art_on: bool):
     import torch
     pin = lambda t: None if t is None else t.cpu().pin_memory()
     q, bt, sl, el, ec = pin(w.q), pin(w.block_table), pin(w.seq_lens), pin(w.eligible_blocks), pin(w.eligible_counts)
-    out = torch.empty((w.batch, w.num_q_heads, w.head_dim), dtype=torch.float32).pin_memory()
+    out = torch.empty(tuple(w.q.shape), dtype=torch.float32).pin_memory()
     stop = torch.empty((w.batch, w.num_kv_heads), dtype=torch.int32).pin_memory()
     desc = art.make_desc(w, eligible_counts=ec)
     ws = torch.empty(art.art_workspace_bytes(desc), dtype=torch.uint8, device=w.q.device)
@@ -378,6 +378,8 @@ def main():
     ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
                     help="time ONLY this arm of one config (short command for ncu captures; prints a small JSON line)")
+    ap.add_argument("--q-len", type=int, default=1, help="--arm only: m query tokens per sequence (SURVEY 8(f).4; m * G <= 8)")
+    ap.add_argument("--q-heads", type=int, default=0, help="--arm only: override the number of query heads (group size G = Hq / Hkv)")
     ap.add_argument("--config", default="1a", help="config for --arm: index + sub, e.g. 1a, 2a, 3a, 3b, 4a, 0a")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "art" else args.warmup
@@ -413,12 +415,15 @@ def main():
 
     if args.arm and args.config != "1a":
         idx, sub = int(args.config[0]), args.config[1:] or "a"
-        wa = gen.config(idx, sub=sub, device=dev, variant="R" if args.arm.startswith("R_") else "")
+        wa = gen.config(idx, sub=sub, device=dev, variant="R" if args.arm.startswith("R_") else "",
+                        **({"num_q_heads": args.q_heads} if args.q_heads else {}))
+        if args.q_len > 1:
+            wa = gen.with_query_tokens(wa, args.q_len, seed=args.q_len)
         torch.cuda.synchronize()
         kw = {"patience": art.ART_PATIENCE_INF} if args.arm == "pinf" else {}
         sp = args.split if wa.dtype == torch.bfloat16 else 0
         r = measure(art, wa, args.steps, args.warmup, None, art_on=args.arm not in ("off", "R_off"), split=sp, **kw)
-        r.update(arm=args.arm, config=wa.name, split=sp or art.art_query_split(art.make_desc(wa), args.arm not in ("off", "R_off")))
+        r.update(arm=args.arm, config=wa.name, q_len=args.q_len, split=sp or art.art_query_split(art.make_desc(wa), args.arm not in ("off", "R_off")))
         print(json.dumps(r), flush=True)
         return
 
@@ -431,10 +436,17 @@ def main():
 
     if args.arm:
         wa = wR if args.arm.startswith("R_") else w
+        if args.q_heads:
+            wa = gen.config(1, device=dev, variant="R" if args.arm.startswith("R_") else "", seed=rank_seed(rank),
+                            num_q_heads=args.q_heads)
+        if args.q_len > 1:
+            wa = gen.with_query_tokens(wa, args.q_len, seed=args.q_len)
         kw = {"patience": art.ART_PATIENCE_INF} if args.arm == "pinf" else {}
         r = measure(art, wa, args.steps, args.warmup, barrier, art_on=args.arm not in ("off", "R_off"),
                     split=args.split, **kw)
         r["arm"] = args.arm
+        r["q_len"] = args.q_len
+        r["q_heads"] = wa.num_q_heads
         r["split"] = args.split or art.art_query_split(art.make_desc(wa), args.arm not in ("off", "R_off"))
         print(json.dumps(r), flush=True)
         return
