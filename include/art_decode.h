@@ -47,7 +47,7 @@ enum {
   ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G = Hq / Hkv > 8, q_len * G > 8, q_len > 1 with ART_SPLIT_DYNAMIC,
                              unsupported head_dim, block_tokens != 64, negative sizes, policy/list mismatch,
                              bad thresholds */
-  ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128; q_len > 1: BF16) */
+  ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128) */
   ART_ERR_ALIGN = -4,     /* q / k_cache / v_cache not 16-byte aligned */
   ART_ERR_WORKSPACE = -5, /* workspace NULL, misaligned or too small where one is needed (the *_host entry point,
                              split == ART_SPLIT_DYNAMIC) */
@@ -89,8 +89,8 @@ typedef struct art_desc {
                                   sequence (their K/V are in the cache and counted in seq_lens); query token i attends
                                   to the eligible tokens j <= L - m + i; the group walks its blocks once and the
                                   criterion is the AND over all m * G (token, head) rows (reading R15).
-                                  m > 1 needs m * G <= 8, BF16 and a cluster schedule (split >= 0); q and out are
-                                  then [B, m, Hq, d]. */
+                                  m > 1 needs m * G <= 8 and a cluster schedule (split >= 0); q and out are then
+                                  [B, m, Hq, d]. */
   const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
   int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
                                   (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */

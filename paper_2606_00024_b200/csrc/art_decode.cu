@@ -175,8 +175,7 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
   const int G = d->num_q_heads / d->num_kv_heads;
   if (G > 8) return ART_ERR_SHAPE;
   if (d->q_len < 0 || d->q_len > 8 || G * qlen_of(d) > 8) return ART_ERR_SHAPE;
-  if (d->q_len > 1) {                                   // built for the bf16 cluster kernel only
-    if (d->dtype == ART_DTYPE_F32) return ART_ERR_DTYPE;
+  if (d->q_len > 1) {                                   // built for the cluster kernels, not for the dynamic scheduler
     if (d->split == ART_SPLIT_DYNAMIC) return ART_ERR_SHAPE;
     if (d->max_blocks_per_seq >= (1 << 24) || d->max_eligible >= (1 << 24)) return ART_ERR_SHAPE;
   }
@@ -632,7 +631,6 @@ int art_query_split(const art_desc_t* desc, int art_on) {
   if (!desc) return ART_ERR_NULL;
   if (desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->num_q_heads % desc->num_kv_heads) return ART_ERR_SHAPE;
   if (desc->num_q_heads / desc->num_kv_heads > 8 || desc->q_len < 0 || art::rows_of(desc) > 8) return ART_ERR_SHAPE;
-  if (desc->q_len > 1 && desc->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;

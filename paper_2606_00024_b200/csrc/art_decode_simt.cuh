@@ -244,11 +244,13 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
     const int half = lane >> 4, c16 = lane & 15;
     float qreg[G][E16];                                      // this lane's 16-byte chunk of every head's q
     {
-      const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * D + c16 * E16;
+      // row h = query token h / Gh, head h % Gh of the group (R15; one query token: row == head)
+      const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.qlen * p.Hq + g * p.Gh) * D + c16 * E16;
 #pragma unroll
       for (int h = 0; h < G; ++h)
 #pragma unroll
-        for (int e = 0; e < E16; ++e) qreg[h][e] = (h < p.Gr) ? to_float(qp[h * D + e]) * p.scale_log2 : 0.f;   // padding heads: q = 0
+        for (int e = 0; e < E16; ++e)                          // padding rows: q = 0
+          qreg[h][e] = (h < p.Gr) ? to_float(qp[((h / p.Gh) * p.Hq + h % p.Gh) * D + e]) * p.scale_log2 : 0.f;
     }
     float pend[G][E8], pend_m[G], pend_l[G];
     bool have_pend = false; int pend_t = 0;
@@ -287,6 +289,9 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
         if (!got) break;
       }
       const unsigned long long vmask = info[stage].mask;
+      // R15: the row this lane ends up with after the reduction may not see the last `cut` tokens of the sequence;
+      // e = tokens of the sequence from the start of this block on (cut == 0 for a single query token)
+      const int row_lim = (L - info[stage].blk * kBlockTokens) - static_cast<int>((p.cuts >> (4 * head_of_lane<G>(lane))) & 15u);
       const uint32_t Kt = sbase + sm.ring + stage * kStageBytes, Vt = Kt + kTileBytes;
 
       // ---- A3: s = q.k / sqrt(d) (log2 domain) for this warp's 8 tokens; lane ends with head hl
@@ -305,7 +310,7 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
           s[h] = a;
         }
         Reduce16<G, 8>::run(s, lane);
-        sv[pp] = ((vmask >> r) & 1ull) ? s[0] : kNegInf;     // masked tokens: weight 0 (R8)
+        sv[pp] = (((vmask >> r) & 1ull) && r < row_lim) ? s[0] : kNegInf;     // masked tokens: weight 0 (R8)
       }
       // ---- A4: block-local softmax over the warp's 8 tokens
       float mloc = fmaxf(fmaxf(sv[0], sv[1]), fmaxf(sv[2], sv[3]));
@@ -540,7 +545,8 @@ __global__ void __launch_bounds__(kThreads, 1) art_decode_kernel(const Params p)
         a = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta[o]), c)), a);
         l = fmaf(f, ld_cluster_f32(mapa(smem_u32(&cta_l[h]), c)), l);
       }
-      if (h < p.Gr) p.out[(static_cast<int64_t>(b) * p.Hq + g * p.Gr) * D + o] = (l > 0.f) ? a / l : 0.f;   // Alg. 1 l.18
+      if (h < p.Gr)                                             // Alg. 1 l.18; row h = query token h / Gh, head h % Gh
+        p.out[((static_cast<int64_t>(b) * p.qlen + h / p.Gh) * p.Hq + g * p.Gh + h % p.Gh) * D + (o - h * D)] = (l > 0.f) ? a / l : 0.f;
     }
     if (tid == 0) {
       if (!ART) p.stop_block[group] = Tn;

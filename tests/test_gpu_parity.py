@@ -434,3 +434,25 @@ def test_multi_token_host_entry():
                                 w.seq_lens.pin_memory(), th, out_h, stop_h, ws)
     rep = compare(w, out_h, stop_h, art=True, oracle_over=dict(tau=f32(1e-3)))
     assert rep.ok(OUT_TOL[w.dtype]) and rep.fired_groups > 0, rep
+
+
+@pytest.mark.parametrize("m,G", [(2, 4), (4, 2), (8, 1), (3, 2), (2, 1)])
+@pytest.mark.parametrize("split", [0, 1, 4])
+def test_multi_token_fp32(m, G, split):
+    """The CUDA-core fp32 kernel (d = 64) takes the same rows and the same causal cut."""
+    kw = dict(num_q_heads=G * 2, num_kv_heads=2, head_dim=64, dtype=torch.float32, planted_frac=0.01, sink_plant=4)
+    w = gen.with_query_tokens(gen.make_workload("multi32", seed=31, batch=2, seq_lens=[1500, 777], **kw), m, seed=m)
+    check(w, art_on=False, split=split)
+    check(w, split=split)
+    wd = gen.with_query_tokens(gen.make_workload("multi32R", seed=32, batch=2, seq_lens=[4096, 3000],
+                                                 recency_decay=(0.2, 1.0), **kw), m, seed=m)
+    check(wd, split=split, tau=1e-3, expect_fired=True)
+
+
+@pytest.mark.parametrize("L", [1, 3, 63, 64, 65, 66, 70, 71, 128, 130])
+def test_multi_token_fp32_block_boundaries(L):
+    for m, G in [(4, 2), (8, 1)]:
+        w = gen.with_query_tokens(gen.make_workload("multi32b", seed=L, batch=2, num_q_heads=G, num_kv_heads=1, head_dim=64,
+                                                    dtype=torch.float32, seq_lens=[L, max(1, L - 1)]), m, seed=L + m)
+        check(w, art_on=False)
+        check(w, tau=1e9, phi=2.5, patience=1)
