@@ -188,6 +188,10 @@ size_t art_workspace_bytes(const art_desc_t* desc);
 /* Cluster size the library would pick for desc->split == 0 (needs a CUDA device); <0 = error code. */
 int art_query_split(const art_desc_t* desc, int art_on);
 
+/* Number of persistent clusters the library would launch for this problem (BF16 only; needs a CUDA device);
+ * art_on: 0 = detector off, 1 = probe of 32 coordinates, 2 = full-output detector.  <0 = error code. */
+int art_query_clusters(const art_desc_t* desc, int art_on);
+
 /* Human-readable text for a status code (static storage). */
 const char* art_status_string(int status);
 

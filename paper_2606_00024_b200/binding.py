@@ -77,6 +77,8 @@ def load_library():
     lib.art_workspace_bytes.argtypes = [C.POINTER(ArtDesc)]
     lib.art_query_split.restype = C.c_int
     lib.art_query_split.argtypes = [C.POINTER(ArtDesc), C.c_int]
+    lib.art_query_clusters.restype = C.c_int
+    lib.art_query_clusters.argtypes = [C.POINTER(ArtDesc), C.c_int]
     lib.art_status_string.restype = C.c_char_p
     lib.art_status_string.argtypes = [C.c_int]
     lib.art_version.restype = C.c_int
@@ -107,8 +109,13 @@ def art_workspace_bytes(desc: ArtDesc) -> int:
     return int(load_library().art_workspace_bytes(C.byref(desc)))
 
 
-def art_query_split(desc: ArtDesc, art_on: bool = True) -> int:
-    return int(load_library().art_query_split(C.byref(desc), int(bool(art_on))))
+def art_query_split(desc: ArtDesc, art_on=True) -> int:
+    """Cluster size the library picks; art_on: False / True / 2 (full-output detector)."""
+    return int(load_library().art_query_split(C.byref(desc), int(art_on)))
+
+
+def art_query_clusters(desc: ArtDesc, art_on=True) -> int:
+    return int(load_library().art_query_clusters(C.byref(desc), int(art_on)))
 
 
 _ws_cache = {}

@@ -1,32 +1,70 @@
-"""Builds libart_decode.so (sm_100a) in-tree with nvcc.  No torch types cross this boundary."""
+"""Builds libart_decode.so (sm_100a) in-tree with nvcc.  No torch types cross this boundary.
+
+Every .cu under csrc/ is one translation unit (the tensor-core kernels are instantiated per group size in their own
+files), compiled in parallel to build/<name>.o and linked into one shared library.
+"""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
-SRC = [os.path.join(HERE, "csrc", "art_decode.cu")]
+CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libart_decode.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-lineinfo", "-gencode", "arch=compute_100a,code=sm_100a",
-         "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include")]
+         "-Xcompiler", "-fPIC", "-I", os.path.join(ROOT, "include")]
 
 
-def needs_build() -> bool:
-    if not os.path.exists(LIB):
-        return True
-    csrc = os.path.join(HERE, "csrc")
-    deps = [os.path.join(csrc, f) for f in os.listdir(csrc)] + [os.path.join(ROOT, "include", "art_decode.h")]
-    return any(os.path.getmtime(d) > os.path.getmtime(LIB) for d in deps)
+def sources() -> list[str]:
+    return sorted(os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith(".cu"))
+
+
+def _headers() -> list[str]:
+    return [os.path.join(CSRC, f) for f in os.listdir(CSRC) if not f.endswith(".cu")] + \
+           [os.path.join(ROOT, "include", "art_decode.h"), os.path.abspath(__file__)]
+
+
+def _flag_stamp(extra: list[str]) -> str:
+    return " ".join(FLAGS + extra)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    if force or needs_build():
-        extra = os.environ.get("ART_NVCC_FLAGS", "").split()      # e.g. -DART_TRACE for a debugging build
-        cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + SRC + ["-o", LIB]
-        subprocess.run(cmd, check=True)
+    extra = os.environ.get("ART_NVCC_FLAGS", "").split()      # e.g. -DART_WATCHDOG for a debugging build
+    os.makedirs(OBJ, exist_ok=True)
+    stamp_path = os.path.join(OBJ, "flags.txt")
+    stamp = _flag_stamp(extra)
+    if not os.path.exists(stamp_path) or open(stamp_path).read() != stamp:
+        force = True
+    hdr_time = max(os.path.getmtime(h) for h in _headers())
+    jobs = []
+    for src in sources():
+        obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+        if force or not os.path.exists(obj) or os.path.getmtime(obj) < max(hdr_time, os.path.getmtime(src)):
+            jobs.append((src, obj))
+
+    def compile_one(job):
+        src, obj = job
+        cmd = [NVCC] + FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        return src, r
+
+    if jobs:
+        with ThreadPoolExecutor(max_workers=min(len(jobs), os.cpu_count() or 4)) as ex:
+            for src, r in ex.map(compile_one, jobs):
+                if verbose or r.returncode != 0:
+                    sys.stderr.write(r.stdout + r.stderr)
+                if r.returncode != 0:
+                    raise subprocess.CalledProcessError(r.returncode, src)
+    objs = [os.path.join(OBJ, os.path.basename(s)[:-3] + ".o") for s in sources()]
+    if jobs or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
+        subprocess.run([NVCC, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB] + objs, check=True)
+    with open(stamp_path, "w") as f:
+        f.write(stamp)
     return LIB
 
 

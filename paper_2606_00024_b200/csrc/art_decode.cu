@@ -12,8 +12,9 @@
 #include <mutex>
 #include <utility>
 #include "art_decode_simt.cuh"
-#include "art_decode_tc.cuh"
-#include "art_decode_ws_kernel.cuh"
+#include "art_decode_pc.cuh"
+#include "art_host_util.cuh"
+#include "art_launch.h"
 #include "art_policy.cuh"
 
 namespace art {
@@ -27,71 +28,6 @@ static inline int qlen_of(const art_desc_t* d) { return d->q_len > 1 ? d->q_len 
 static inline int rows_of(const art_desc_t* d) { return (d->num_q_heads / d->num_kv_heads) * qlen_of(d); }
 
 struct LaunchPlan { int C, stages, mslots; uint32_t smem; };
-
-static void set_cluster_attr(cudaLaunchAttribute* attr, int C) {
-  attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = C; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-}
-
-template <typename Kern> static cudaError_t prepare_kernel_uncached(Kern kern, int C, uint32_t smem_bytes);
-// The attribute calls cost a few microseconds each on the host.  They are per-function state, so what has been set
-// is remembered per (device, kernel): the dynamic shared memory limit only ever grows (a larger limit than a launch
-// needs is harmless), the carveout preference and the non-portable cluster size are set once.
-template <typename Kern>
-static cudaError_t prepare_kernel(Kern kern, int C, uint32_t smem_bytes) {
-  struct State { uint32_t smem = 0; bool nonportable = false; };
-  static std::mutex mu;
-  static std::map<std::array<uintptr_t, 2>, State> done;
-  int dev = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess) return cudaGetLastError();
-  const std::array<uintptr_t, 2> key = {static_cast<uintptr_t>(dev), reinterpret_cast<uintptr_t>(kern)};
-  std::lock_guard<std::mutex> lock(mu);
-  State& st = done[key];
-  if (st.smem >= smem_bytes && (C <= 8 || st.nonportable)) return cudaSuccess;
-  const uint32_t want = smem_bytes > st.smem ? smem_bytes : st.smem;
-  cudaError_t e = prepare_kernel_uncached(kern, C > 8 || st.nonportable ? 16 : 1, want);
-  if (e == cudaSuccess) { st.smem = want; st.nonportable = st.nonportable || C > 8; }
-  return e;
-}
-template <typename Kern>
-static cudaError_t prepare_kernel_uncached(Kern kern, int C, uint32_t smem_bytes) {
-  cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, static_cast<int>(smem_bytes));
-  if (e != cudaSuccess) return e;
-  // two CTAs per SM need the whole unified L1/shared array configured as shared memory
-  e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, static_cast<int>(cudaSharedmemCarveoutMaxShared));
-  if (e != cudaSuccess) return e;
-  if (C > 8) e = cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1);
-  return e;
-}
-
-template <typename Kern, typename... Args>
-static cudaError_t launch_cluster(Kern kern, int threads, int groups, int C, uint32_t smem_bytes, cudaStream_t stream,
-                                  Args... args) {
-  cudaError_t e = prepare_kernel(kern, C, smem_bytes);
-  if (e != cudaSuccess) return e;
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(static_cast<unsigned>(groups) * C, 1, 1);
-  cfg.blockDim = dim3(threads, 1, 1);
-  cfg.dynamicSmemBytes = smem_bytes;
-  cfg.stream = stream;
-  cudaLaunchAttribute attr[1];
-  set_cluster_attr(attr, C);
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  return cudaLaunchKernelEx(&cfg, kern, args...);
-}
-
-template <typename Kern>
-static int max_active_clusters(Kern kern, int threads, int C, uint32_t smem_bytes) {
-  if (prepare_kernel(kern, C, smem_bytes) != cudaSuccess) { cudaGetLastError(); return 0; }
-  cudaLaunchConfig_t cfg = {};
-  cfg.gridDim = dim3(C, 1, 1); cfg.blockDim = dim3(threads, 1, 1); cfg.dynamicSmemBytes = smem_bytes;
-  cudaLaunchAttribute attr[1];
-  set_cluster_attr(attr, C);
-  cfg.attrs = attr; cfg.numAttrs = 1;
-  int n = 0;
-  if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
-  return n;
-}
 
 // dispatch over (G, MODE) with a generic functor f(mode_constant, G_constant)
 template <typename F>
@@ -175,10 +111,7 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
   const int G = d->num_q_heads / d->num_kv_heads;
   if (G > 8) return ART_ERR_SHAPE;
   if (d->q_len < 0 || d->q_len > 8 || G * qlen_of(d) > 8) return ART_ERR_SHAPE;
-  if (d->q_len > 1) {                                   // built for the cluster kernels, not for the dynamic scheduler
-    if (d->split == ART_SPLIT_DYNAMIC) return ART_ERR_SHAPE;
-    if (d->max_blocks_per_seq >= (1 << 24) || d->max_eligible >= (1 << 24)) return ART_ERR_SHAPE;
-  }
+  if (d->dtype == ART_DTYPE_BF16 && (d->max_blocks_per_seq >= (1 << 24) || d->max_eligible >= (1 << 24))) return ART_ERR_SHAPE;   // a step number is 24 bits
   if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
   if (d->dtype != ART_DTYPE_F32 && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (d->head_dim != 64 && d->head_dim != 128) return ART_ERR_SHAPE;
@@ -190,8 +123,9 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
     if (d->max_eligible < 0) return ART_ERR_SHAPE;
   }
   if (d->policy == ART_POLICY_SINK_WINDOW && (d->sink_tokens < 0 || d->window_tokens < 0)) return ART_ERR_SHAPE;
-  if (d->split < ART_SPLIT_DYNAMIC || d->split > 16) return ART_ERR_SHAPE;
-  if (d->split == ART_SPLIT_DYNAMIC && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
+  const bool legacy = d->split <= -100 && d->split >= -116;
+  if ((d->split < ART_SPLIT_DYNAMIC && !legacy) || d->split > 16) return ART_ERR_SHAPE;
+  if ((d->split == ART_SPLIT_DYNAMIC || legacy) && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (d->dtype == ART_DTYPE_F32 && d->split > 0 && (d->split & (d->split - 1))) return ART_ERR_SHAPE;
   if (!(d->sm_scale >= 0.f) || isinf(d->sm_scale)) return ART_ERR_SHAPE;
   if (th) {
@@ -218,13 +152,16 @@ static int mode_of(const art_desc_t* d, const art_thresholds_t* th) {
   return (th->probe_dim == 0 || th->probe_dim == d->head_dim) ? 2 : 1;
 }
 
-// shared-memory plan for a cluster size
+// ---- which bf16 kernel a descriptor selects.  split = 0 / ART_SPLIT_DYNAMIC / 1..16: persistent clusters (of that
+// size); split = -(100 + C): the static-cluster kernel of round 1 with C CTAs per group (C = 0: its own choice).
+static inline bool legacy_split(const art_desc_t* d) { return d->split <= -100; }
+static inline int legacy_c(const art_desc_t* d) { return -d->split - 100; }
+
+// shared-memory plan of the static-cluster kernels (fp32 CUDA-core kernel; legacy bf16 kernel)
 static LaunchPlan plan_for(bool tensor_core, int G, int PW, bool art, int C) {
   LaunchPlan pl;
   pl.C = C;
   if (tensor_core) {
-    // Two CTAs per SM (3-stage ring each) unless the probe is the full output (MODE 2: bigger mailbox rows,
-    // more registers in the scan warp), which runs one CTA per SM with a deeper ring.
     const bool two_per_sm = !art || PW == 32;
     const uint32_t budget = two_per_sm ? kSmemTwoPerSm : static_cast<uint32_t>(kMaxSmem);
     pl.stages = two_per_sm ? 3 : tc::kMaxStages;
@@ -243,6 +180,23 @@ static LaunchPlan plan_for(bool tensor_core, int G, int PW, bool art, int C) {
   return pl;
 }
 
+// shared-memory plan of the persistent-cluster kernel: two CTAs per SM (3-stage ring each) unless the probe is the
+// full output (MODE 2: 4x larger summaries), which runs one CTA per SM with a deeper ring
+struct PcPlan { int stages, nsum, per_sm; uint32_t smem; };
+static PcPlan plan_pc(int G, int PW, bool art) {
+  PcPlan pl;
+  const bool two_per_sm = !art || PW == 32;
+  const uint32_t budget = two_per_sm ? kSmemTwoPerSm : static_cast<uint32_t>(kMaxSmem);
+  pl.per_sm = two_per_sm ? 2 : 1;
+  pl.stages = two_per_sm ? 3 : tc::kMaxStages;
+  pl.nsum = art ? tc::kPVSlots : 0;
+  auto total = [&]() { return pc::make_smem_map_p(G, PW, pl.stages, pl.nsum, art).total; };
+  while (art && pl.nsum > 2 && total() > budget) pl.nsum >>= 1;      // 8 -> 4 summary slots (G = 8)
+  while (pl.stages > 2 && total() > budget) --pl.stages;
+  pl.smem = total();
+  return pl;
+}
+
 // The occupancy calculator counts a kernel that allocates tensor memory as one CTA per SM, whatever it
 // allocates; the hardware runs two of ours side by side (256 of the SM's 512 columns each; checked with a
 // timestamp probe).  This twin has the same launch shape and no tcgen05 code: it is only ever passed to the
@@ -252,24 +206,31 @@ __global__ void __launch_bounds__(tc::kThreads, 2) tc_occupancy_twin(int* sink) 
   if (sink) *sink = twin_smem[0];
 }
 
+static int occupancy_tc(int G, int mode, int C, uint32_t smem) {
+  switch (G) { case 1: return occupancy_tc_g1(mode, C, smem); case 2: return occupancy_tc_g2(mode, C, smem);
+               case 4: return occupancy_tc_g4(mode, C, smem); default: return occupancy_tc_g8(mode, C, smem); }
+}
+static int occupancy_pc(int G, int mode, int C, uint32_t smem) {
+  switch (G) { case 1: return occupancy_pc_g1(mode, C, smem); case 2: return occupancy_pc_g2(mode, C, smem);
+               case 4: return occupancy_pc_g4(mode, C, smem); default: return occupancy_pc_g8(mode, C, smem); }
+}
+
 // clusters of size C that can be co-resident, cached per (device, kernel class, shared memory size)
-static int cluster_capacity(const art_desc_t* d, int G, int mode, int C, uint32_t smem) {
+// kind: 0 = fp32 CUDA-core kernel, 1 = legacy bf16 kernel, 2 = persistent-cluster kernel
+static int cluster_capacity(int kind, int G, int mode, int C, uint32_t smem) {
   static std::mutex mu;
   static std::map<std::array<int, 4>, int> cache;
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return 0; }
-  const bool tensor_core = d->dtype == ART_DTYPE_BF16;
-  const bool twin = tensor_core && mode != 2;
-  const std::array<int, 4> key = {dev, twin ? -1 : (tensor_core ? 100 : 0) + G * 4 + mode, C, static_cast<int>(smem)};
+  const bool twin = kind != 0 && mode != 2;
+  const std::array<int, 4> key = {dev, twin ? -1 : kind * 100 + G * 4 + mode, C, static_cast<int>(smem)};
   std::lock_guard<std::mutex> lock(mu);
   auto it = cache.find(key);
   if (it != cache.end()) return it->second;
   int fit;
   if (twin) fit = max_active_clusters(tc_occupancy_twin, tc::kThreads, C, smem);
-  else if (tensor_core)
-    fit = dispatch(G, mode, [&](auto m, auto gg) {
-      return max_active_clusters(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value>, tc::kThreads, C, smem);
-    });
+  else if (kind == 1) fit = occupancy_tc(G, mode, C, smem);
+  else if (kind == 2) fit = occupancy_pc(G, mode, C, smem);
   else
     fit = dispatch(G, mode, [&](auto m, auto gg) {
       return max_active_clusters(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>, simt::kThreads, C, smem);
@@ -278,16 +239,15 @@ static int cluster_capacity(const art_desc_t* d, int G, int mode, int C, uint32_
   return fit;
 }
 
-// Cluster size: the largest C (<= 16) whose clusters for ALL groups can be co-resident, so every
-// group streams from the first cycle; never more CTAs than a group could have blocks.  The tensor-core
-// kernel takes any C (steps are dealt round-robin); the CUDA-core kernel's mailbox wants a power of two.
-static int choose_split(const art_desc_t* d, int mode, int* C_out) {
+// Static-cluster kernels: the largest C (<= 16) whose clusters for ALL groups can be co-resident, so every
+// group streams from the first cycle; never more CTAs than a group could have blocks.
+static int choose_split(const art_desc_t* d, int mode, int want, int* C_out) {
   const int G = padded_group(rows_of(d));
   const int groups = d->batch * d->num_kv_heads;
   const bool art = mode != 0;
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
-  if (d->split != 0) { *C_out = d->split; return ART_OK; }
+  if (want != 0) { *C_out = want; return ART_OK; }
   int maxT = d->policy == ART_POLICY_LIST ? d->max_eligible : d->max_blocks_per_seq;
   if (d->policy == ART_POLICY_SINK_WINDOW) {
     const int sw = (d->sink_tokens + 63) / 64 + (d->window_tokens + 63) / 64 + 1;
@@ -298,50 +258,59 @@ static int choose_split(const art_desc_t* d, int mode, int* C_out) {
     if (C > maxT) continue;
     if (!tensor_core && (C & (C - 1))) continue;
     const LaunchPlan pl = plan_for(tensor_core, G, PW, art, C);
-    const int fit = cluster_capacity(d, G, mode, C, pl.smem);
+    const int fit = cluster_capacity(tensor_core ? 1 : 0, G, mode, C, pl.smem);
     if (fit >= groups && fit > 0) { best = C; break; }
   }
   *C_out = best;
   return ART_OK;
 }
 
-
-// ---- dynamically scheduled kernel (art_decode_ws_kernel.cuh): launch plan
-struct WsPlan { int stages, ms, per_sm; uint32_t smem; };
-static WsPlan plan_ws(int G, int PW, bool art) {
-  WsPlan pl;
-  pl.per_sm = 2; pl.stages = 3; pl.ms = art ? 16 : 0;      // staging window: a power of two, at most 16
-  auto total = [&]() { return ws::make_smem_map_w(G, PW, pl.stages, pl.ms, art).total; };
-  if (total() <= kSmemTwoPerSm) { pl.smem = total(); return pl; }
-  // does not fit twice: one CTA per SM with a deeper ring and a full staging window
-  pl.per_sm = 1; pl.stages = tc::kMaxStages; pl.ms = art ? 16 : 0;
-  while (pl.stages > 2 && total() > static_cast<uint32_t>(kMaxSmem)) --pl.stages;
-  pl.smem = total();
-  return pl;
-}
-
-static int sm_count() {
-  int dev = 0, n = 0;
-  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
-    cudaGetLastError(); return 0;
+// Persistent clusters: cluster size CL (the caller's, else the largest of 16, 8, 4, 2, 1 that the device can
+// co-schedule at all) and the number of clusters NC = min(co-resident clusters, groups).
+static int choose_pc(int G, int mode, int want, int groups, const PcPlan& pl, int* CL_out, int* NC_out) {
+  int CL = want > 0 ? want : 16, fit = 0;
+  for (;;) {
+    fit = cluster_capacity(2, G, mode, CL, pl.smem);
+    if (fit > 0 || want > 0 || CL == 1) break;
+    CL >>= 1;
   }
-  return n;
+  if (fit <= 0) return ART_ERR_CUDA;
+  *CL_out = CL; *NC_out = fit < groups ? fit : groups;
+  return ART_OK;
 }
 
-// workspace the dynamically scheduled kernel needs (worst case over the probe widths)
+// run-ahead per worker of the persistent-cluster kernel (steps whose loads may be issued beyond the last decided
+// step, per CTA working on the group); ART_PC_RUNAHEAD overrides it for measurements
+static int pc_run_ahead(int nsum) {
+  static const int env = [] { const char* e = getenv("ART_PC_RUNAHEAD"); return e ? atoi(e) : 0; }();
+  int rw = env > 0 ? env : 6;
+  return rw;
+}
+
+#ifdef ART_WATCHDOG
+// debugging build: a pinned, device-mapped word that a wait which never ends writes before it traps; it survives
+// the death of the context, so the test harness can print where the kernel was stuck (art_debug_watchdog())
+static unsigned long long* g_watchdog_host = nullptr;
+static unsigned long long* watchdog_word() {
+  static unsigned long long* dev = [] {
+    unsigned long long* h = nullptr; unsigned long long* dptr = nullptr;
+    if (cudaHostAlloc(&h, 64, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return dptr; }
+    h[0] = 0ull;
+    if (cudaHostGetDevicePointer(&dptr, h, 0) != cudaSuccess) { cudaGetLastError(); return static_cast<unsigned long long*>(nullptr); }
+    g_watchdog_host = h;
+    return dptr;
+  }();
+  return dev;
+}
+#endif
+
+// workspace of the persistent-cluster kernel: one partial state (m, l, acc) per (group, CTA of a cluster)
+static size_t pc_part_bytes(int groups, int G) {
+  return static_cast<size_t>(groups) * pc::kMaxCL * static_cast<size_t>(G * (tc::kD + 2)) * 4u;
+}
 static size_t ws_bytes_for(const art_desc_t* d) {
-  if (d->dtype != ART_DTYPE_BF16 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads || d->num_q_heads / d->num_kv_heads > 8) return 0;
-  const int G = padded_group(d->num_q_heads / d->num_kv_heads);
-  return ws::make_ws_layout(d->batch * d->num_kv_heads, G, d->head_dim, true).total;
-}
-
-template <typename Kern>
-static cudaError_t launch_ws(Kern kern, int grid, uint32_t smem_bytes, cudaStream_t stream, const Params& p,
-                             const ws::WsView& v, const CUtensorMap& tmK, const CUtensorMap& tmV) {
-  cudaError_t e = prepare_kernel(kern, 1, smem_bytes);
-  if (e != cudaSuccess) return e;
-  kern<<<grid, tc::kThreads, smem_bytes, stream>>>(p, v, tmK, tmV);
-  return cudaGetLastError();
+  if (d->dtype != ART_DTYPE_BF16 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads || rows_of(d) > 8) return 0;
+  return pc_part_bytes(d->batch * d->num_kv_heads, padded_group(rows_of(d))) + 256;
 }
 
 static int run(const art_desc_t* d, const void* q, const void* k, const void* v, const int32_t* bt,
@@ -354,11 +323,7 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
-  const bool dynamic = tensor_core && d->split == ART_SPLIT_DYNAMIC;   // persistent grid, steps claimed at run time
-  int C = 1;
-  int rc = dynamic ? ART_OK : choose_split(d, mode, &C);
-  if (rc != ART_OK) return rc;
-  const LaunchPlan pl = dynamic ? LaunchPlan{1, 0, 0, 0u} : plan_for(tensor_core, G, PW, mode != 0, C);
+  const bool persistent = tensor_core && !legacy_split(d);
 
   Params p = {};
   p.q = q; p.k = static_cast<const uint8_t*>(k); p.v = static_cast<const uint8_t*>(v);
@@ -378,48 +343,66 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const float scale = d->sm_scale > 0.f ? d->sm_scale : 1.0f / sqrtf(static_cast<float>(d->head_dim));
   p.scale_log2 = scale * 1.4426950408889634f;
   if (th) { p.tau = th->tau; p.phi = th->phi; p.patience = th->patience; }
-  p.stages = pl.stages; p.mbox_slots = pl.mslots;
-  // With the detector on, the CTAs of a cluster are coupled through the mailbox window; claiming steps at run time
-  // keeps a CTA that shares its SM from holding the others back.  It pays for clusters of 2-4 (measured).
-  p.dyn = (tensor_core && mode != 0 && C >= 2 && C <= 4) ? 1 : 0;
 
   cudaError_t e;
-  if (dynamic) {
-    ws::WsLayout lay = ws::make_ws_layout(groups, G, PW, mode != 0);
-    if (!workspace || workspace_bytes < lay.total || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return ART_ERR_WORKSPACE;
-    lay.v.base = static_cast<uint8_t*>(workspace);
-    const WsPlan wp = plan_ws(G, PW, mode != 0);
-    p.stages = wp.stages; p.mbox_slots = wp.ms;
-    const int sms = sm_count();
-    if (sms <= 0) return ART_ERR_CUDA;
-    CUtensorMap tmK, tmV;
-    if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
-      return ART_ERR_CUDA;
-    if (cudaMemsetAsync(workspace, 0, lay.zero_bytes, stream) != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
-    if (blocks_loaded && cudaMemsetAsync(blocks_loaded, 0, sizeof(int32_t) * groups, stream) != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
-    e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
-      return static_cast<int>(launch_ws(ws::art_decode_ws_kernel<decltype(gg)::value, decltype(m)::value>,
-                                        sms * wp.per_sm, wp.smem, stream, p, lay.v, tmK, tmV));
-    }));
-  } else if (tensor_core) {
-#ifdef ART_TRACE
-    if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
+  if (persistent) {
+    const PcPlan pl = plan_pc(G, PW, mode != 0);
+    int CL = 1, NC = 1;
+    int rc = choose_pc(G, mode, d->split > 0 ? d->split : 0, groups, pl, &CL, &NC);
+    if (rc != ART_OK) return rc;
+    const size_t need = pc_part_bytes(groups, G);
+    if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return ART_ERR_WORKSPACE;
+    p.stages = pl.stages; p.mbox_slots = 0; p.dyn = 1;
+    pc::PcParams pp = {};
+    pp.b = p; pp.n_groups = groups; pp.NC = NC; pp.part = static_cast<float*>(workspace);
+    pp.rw = pc_run_ahead(pl.nsum); pp.nsum = pl.nsum > 0 ? pl.nsum : 1;
+    pp.dbg = nullptr;
+#ifdef ART_WATCHDOG
+    pp.dbg = watchdog_word();
 #endif
     CUtensorMap tmK, tmV;
     if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
       return ART_ERR_CUDA;
-    e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
-      if (p.qlen > 1)
-        return static_cast<int>(launch_cluster(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value, true>,
-                                               tc::kThreads, groups, C, pl.smem, stream, p, tmK, tmV));
-      return static_cast<int>(launch_cluster(tc::art_decode_tc_kernel<decltype(gg)::value, decltype(m)::value>,
-                                             tc::kThreads, groups, C, pl.smem, stream, p, tmK, tmV));
-    }));
+    if (blocks_loaded && cudaMemsetAsync(blocks_loaded, 0, sizeof(int32_t) * groups, stream) != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
+    const bool mt = p.qlen > 1;
+    int r;
+    switch (G) {
+      case 1: r = launch_pc_g1(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      case 2: r = launch_pc_g2(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      case 4: r = launch_pc_g4(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      default: r = launch_pc_g8(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+    }
+    e = static_cast<cudaError_t>(r);
   } else {
-    e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
-      return static_cast<int>(launch_cluster(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>,
-                                             simt::kThreads, groups, C, pl.smem, stream, p));
-    }));
+    int C = 1;
+    int rc = choose_split(d, mode, tensor_core ? legacy_c(d) : d->split, &C);
+    if (rc != ART_OK) return rc;
+    const LaunchPlan pl = plan_for(tensor_core, G, PW, mode != 0, C);
+    p.stages = pl.stages; p.mbox_slots = pl.mslots;
+    // legacy bf16 kernel: with the detector on, steps are claimed at run time for clusters of 2-4 (measured in round 1)
+    p.dyn = (tensor_core && mode != 0 && C >= 2 && C <= 4) ? 1 : 0;
+    if (tensor_core) {
+#ifdef ART_TRACE
+      if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
+#endif
+      CUtensorMap tmK, tmV;
+      if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
+        return ART_ERR_CUDA;
+      const bool mt = p.qlen > 1;
+      int r;
+      switch (G) {
+        case 1: r = launch_tc_g1(mode, mt, groups, C, pl.smem, stream, p, tmK, tmV); break;
+        case 2: r = launch_tc_g2(mode, mt, groups, C, pl.smem, stream, p, tmK, tmV); break;
+        case 4: r = launch_tc_g4(mode, mt, groups, C, pl.smem, stream, p, tmK, tmV); break;
+        default: r = launch_tc_g8(mode, mt, groups, C, pl.smem, stream, p, tmK, tmV); break;
+      }
+      e = static_cast<cudaError_t>(r);
+    } else {
+      e = static_cast<cudaError_t>(dispatch(G, mode, [&](auto m, auto gg) {
+        return static_cast<int>(launch_cluster(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>,
+                                               simt::kThreads, groups, C, pl.smem, stream, p));
+      }));
+    }
   }
   if (e != cudaSuccess) { cudaGetLastError(); return ART_ERR_CUDA; }
   return ART_OK;
@@ -634,10 +617,32 @@ int art_query_split(const art_desc_t* desc, int art_on) {
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;
-  if (desc->split == ART_SPLIT_DYNAMIC) return 0;                    // dynamic scheduler: no fixed cluster
+  const int mode = art_on == 2 ? 2 : (art_on ? 1 : 0);                 // 2: detector on the full output (probe_dim = 0 or d)
   int C = 1;
-  rc = art::choose_split(desc, art_on ? 1 : 0, &C);
+  if (desc->dtype == ART_DTYPE_BF16 && !art::legacy_split(desc)) {
+    const int G = art::padded_group(art::rows_of(desc));
+    const art::PcPlan pl = art::plan_pc(G, mode == 2 ? desc->head_dim : 32, mode != 0);
+    int NC = 1;
+    rc = art::choose_pc(G, mode, desc->split > 0 ? desc->split : 0, desc->batch * desc->num_kv_heads > 0 ? desc->batch * desc->num_kv_heads : 1, pl, &C, &NC);
+    return rc == ART_OK ? C : rc;
+  }
+  rc = art::choose_split(desc, mode, desc->dtype == ART_DTYPE_BF16 ? art::legacy_c(desc) : desc->split, &C);
   return rc == ART_OK ? C : rc;
+}
+
+int art_query_clusters(const art_desc_t* desc, int art_on) {
+  if (!desc) return ART_ERR_NULL;
+  if (desc->dtype != ART_DTYPE_BF16 || art::legacy_split(desc)) return ART_ERR_DTYPE;
+  if (desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->num_q_heads % desc->num_kv_heads || art::rows_of(desc) > 8) return ART_ERR_SHAPE;
+  int rc = art::check_arch();
+  if (rc != ART_OK) return rc;
+  const int mode = art_on == 2 ? 2 : (art_on ? 1 : 0);
+  const int G = art::padded_group(art::rows_of(desc));
+  const art::PcPlan pl = art::plan_pc(G, mode == 2 ? desc->head_dim : 32, mode != 0);
+  int CL = 1, NC = 1;
+  const int groups = desc->batch * desc->num_kv_heads;
+  rc = art::choose_pc(G, mode, desc->split > 0 ? desc->split : 0, groups > 0 ? groups : 1, pl, &CL, &NC);
+  return rc == ART_OK ? NC : rc;
 }
 
 const char* art_status_string(int status) {
@@ -655,5 +660,9 @@ const char* art_status_string(int status) {
 }
 
 int art_version(void) { return ART_VERSION; }
+
+#ifdef ART_WATCHDOG
+unsigned long long art_debug_watchdog(void) { return art::g_watchdog_host ? art::g_watchdog_host[0] : 0ull; }
+#endif
 
 }  // extern "C"

@@ -1,0 +1,944 @@
+// ART decode attention, bf16 KV / head_dim 128: PERSISTENT CLUSTERS with run-time scheduling (tcgen05 + TMEM + TMA).
+//
+// The grid is NC thread-block clusters of CL CTAs (CL up to 16, two CTAs per SM), launched once and resident for the
+// whole call.  Cluster c owns the query groups c, c + NC, c + 2 NC, ...  Nothing inside a cluster is bound:
+//
+//   * a CTA that needs work OPENS the next group of its cluster (it becomes the group's HOME: its scan warp replays
+//     Algorithm 1 for the group) or, when the cluster has no unopened group left, JOINS the open group of its cluster
+//     with the most remaining steps per worker.  CTAs freed by a group that terminated early therefore stream for the
+//     groups that still run, and the last long group of a cluster is served by all CL CTAs;
+//   * traversal steps t = 1..T are CLAIMED one at a time from the group's counter on the cluster's
+//     board (rank 0's shared memory, atom.shared::cluster); with the detector on, the TMA loads of step t are issued
+//     only once step t - R has been decided, R = run-ahead per worker x workers: this bounds the blocks that are
+//     loaded and then discarded when Algorithm 1 fires (A7) to the blocks in flight;
+//   * one 64-token KV block is one pipeline ITEM, handled by specialised warps that meet through mbarriers exactly as
+//     in art_decode_tc.cuh (TMA -> S = K Q^T -> block-local softmax -> P~V = V^T P^T with P split hi + lo), its
+//     block-local result waiting UNFOLDED in tensor memory until the decision for its step is known;
+//   * the step summary (m_t, l_t, probe of P~V_t) stays in the shared memory of the CTA that computed it; the home's
+//     scan warp is told where (one word per step, st.shared::cluster) and PULLS it over distributed shared memory.
+//     Every word of a summary carries, in its lowest mantissa bit, the parity of the slot's generation, so the reader
+//     needs no fence: a word is either the previous generation's or final (a 4-byte store is single-copy atomic);
+//   * the scan warp (art_scan_chunk.cuh) decides up to 8 steps per chunk and broadcasts the progress word to the
+//     cluster; fold warps merge P~V_t into the CTA's partial state for t <= t* only, drop the others;
+//   * a CTA that leaves a group flushes its partial (m, l, acc) to the workspace; whoever completes the count of
+//     folded steps combines the partial states (flash-decoding merge) and writes `out` (A8/A9).
+//
+// Steps beyond t* are never folded and the scan consumes summaries in step order whoever computed them, so the
+// result is the sequential algorithm's for any CL and any schedule.  Deadlock freedom: DESIGN.md section 6.
+#pragma once
+#include "art_decode_tc.cuh"
+#include "art_scan_chunk.cuh"
+
+namespace art {
+namespace pc {
+
+using namespace tc;
+
+constexpr int kMaxCL = 16;
+constexpr int kHS = 2 * kMaxCL;              // home slots of a cluster: two per CTA (a CTA opens its next group while the last one drains)
+constexpr int kNR = 64;                      // notice ring per home slot; the run-ahead window never exceeds it
+constexpr int kItemsRing = 32;               // item descriptors; >= stages + kPVSlots + the four END items
+constexpr int kLock = -(1 << 20);            // board.nact while a slot is being (re)opened
+constexpr int kMinJoin = 4;                  // a group with fewer unclaimed steps is not worth a Q reload and a partial state
+static_assert(kItemsRing >= kPVSlots + kMaxStages + 4, "item ring too short");
+
+struct PcParams {
+  Params b;
+  int32_t n_groups, NC;
+  float* part;                               // workspace: partial states [group][rank][G * (kD + 2)]
+  int32_t rw;                                // run-ahead per worker (steps issued beyond the last decided one)
+  int32_t nsum;                              // summary slots per CTA (<= kPVSlots)
+  unsigned long long* dbg;                   // ART_WATCHDOG: where a wait that never ended reports itself
+};
+
+enum { ITEM_DATA = 0, ITEM_FLUSH = 1, ITEM_END = 2 };
+// meta: bits 0-4 home slot, 5 Q buffer, 6-7 kind, 8-14 generation of the slot's group
+struct Item { int tcode; int meta; unsigned long long mask; };   // FLUSH: tcode = blocks loaded in the visit, mask = group
+__device__ __forceinline__ int item_hs(int meta) { return meta & 31; }
+__device__ __forceinline__ int item_q(int meta) { return (meta >> 5) & 1; }
+__device__ __forceinline__ int item_kind(int meta) { return (meta >> 6) & 3; }
+__device__ __forceinline__ int item_gen(int meta) { return (meta >> 8) & 127; }
+
+// progress word of a home slot, broadcast to every CTA of the cluster: [gen:7][fired:1][t:24]
+__device__ __forceinline__ int ctrl_word(int gen, bool fired, int t) { return (gen << 25) | (fired ? (1 << 24) : 0) | t; }
+
+struct BoardEntry { int next, T, nact, group, gen, pad0, pad1, pad2; };        // rank 0: one per home slot
+struct HomeInfo { unsigned long long done; int group, T, gen, loaded; unsigned joined; int pad; };   // home CTA: one per local slot
+
+struct SmemMapP {
+  uint32_t qb, pb, slots, items, sums, tags, hinfo, ctrl, board, bars, misc, ring, total;
+  uint32_t full0, empty0, pfull0, sfull0, sfree0, pvfull0, pvfree0, done0, nbars;
+};
+// summary of one step: [G * PW] probe values (lane l of the scan warp owns floats l*CPL .. l*CPL + CPL - 1), then (m, l) x G
+__host__ __device__ constexpr uint32_t sum_bytes(int G, int PW) { return static_cast<uint32_t>(G * (PW + 2) * 4); }
+
+__host__ __device__ inline SmemMapP make_smem_map_p(int G, int PW, int stages, int nsum, bool art) {
+  SmemMapP m;
+  uint32_t off = 0;
+  m.qb = off; off += 2u * kQBytes;
+  m.pb = off; off += static_cast<uint32_t>(p_bufs(G, stages, art && PW == 32)) * 2u * p_buf_bytes(G);
+  m.slots = off; off += kIterSlots * static_cast<uint32_t>(sizeof(IterSlot));
+  m.items = off; off += kItemsRing * static_cast<uint32_t>(sizeof(Item));
+  off = (off + 15u) & ~15u;
+  m.sums = off; off += art ? static_cast<uint32_t>(nsum) * sum_bytes(G, PW) : 0u;
+  m.tags = off; off += art ? 2u * kNR * 4u : 0u;
+  off = (off + 15u) & ~15u;
+  m.hinfo = off; off += 2u * static_cast<uint32_t>(sizeof(HomeInfo));
+  m.ctrl = off; off += kHS * 4u;
+  m.board = off; off += kHS * static_cast<uint32_t>(sizeof(BoardEntry)) + 16u;    // + next_local
+  m.bars = off;
+  uint32_t n = 0;
+  m.full0 = n; n += stages; m.empty0 = n; n += stages; m.pfull0 = n; n += stages;
+  m.sfull0 = n; n += kSSlots; m.sfree0 = n; n += kSSlots;
+  m.pvfull0 = n; n += kPVSlots; m.pvfree0 = n; n += kPVSlots;
+  m.done0 = n; n += 2;
+  m.nbars = n;
+  off += n * 8u;
+  m.misc = off; off += 32u + 4u * kPVSlots;
+  off = (off + 1023u) & ~1023u;
+  if (off < static_cast<uint32_t>(kFront)) off = kFront;
+  m.ring = off; off += static_cast<uint32_t>(stages) * kStageBytes;
+  m.total = off;
+  return m;
+}
+constexpr uint32_t kMTmem = 0, kMOpen = 4, kMScanExit = 8, kMFlag = 12, kMJoined = 16, kMPubCnt = 32;   // + kPVSlots publish counters
+
+// ----------------------------------------------------------------------------- small PTX helpers
+
+__device__ __forceinline__ int atom_add_cluster(uint32_t a, int v) {           // relaxed
+  int r; asm volatile("atom.relaxed.cluster.shared::cluster.add.s32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
+}
+__device__ __forceinline__ int atom_add_cluster_acqrel(uint32_t a, int v) {
+  int r; asm volatile("atom.acq_rel.cluster.shared::cluster.add.s32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
+}
+__device__ __forceinline__ int atom_cas_cluster_acqrel(uint32_t a, int cmp, int v) {
+  int r; asm volatile("atom.acq_rel.cluster.shared::cluster.cas.b32 %0, [%1], %2, %3;" : "=r"(r) : "r"(a), "r"(cmp), "r"(v) : "memory"); return r;
+}
+__device__ __forceinline__ unsigned atom_or_cluster(uint32_t a, unsigned v) {
+  unsigned r; asm volatile("atom.relaxed.cluster.shared::cluster.or.b32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
+}
+__device__ __forceinline__ unsigned long long atom_add64_cluster_acqrel(uint32_t a, unsigned long long v) {
+  unsigned long long r;
+  asm volatile("atom.acq_rel.cluster.shared::cluster.add.u64 %0, [%1], %2;" : "=l"(r) : "r"(a), "l"(v) : "memory"); return r;
+}
+__device__ __forceinline__ int ld_cluster_relaxed_s32(uint32_t a) {
+  int v; asm volatile("ld.relaxed.cluster.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v;
+}
+__device__ __forceinline__ int ld_cluster_acquire_s32(uint32_t a) {
+  int v; asm volatile("ld.acquire.cluster.shared::cluster.s32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v;
+}
+__device__ __forceinline__ uint32_t ld_cluster_u32(uint32_t a) {
+  uint32_t v; asm volatile("ld.relaxed.cluster.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(a) : "memory"); return v;
+}
+template <int N> __device__ __forceinline__ void ld_cluster_vec(uint32_t a, uint32_t (&r)[N]) {
+  if constexpr (N == 1) {
+    asm volatile("ld.relaxed.cluster.shared::cluster.u32 %0, [%1];" : "=r"(r[0]) : "r"(a) : "memory");
+  } else if constexpr (N == 2) {
+    asm volatile("ld.relaxed.cluster.shared::cluster.v2.u32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(a) : "memory");
+  } else {
+    static_assert(N % 4 == 0, "vector width");
+#pragma unroll
+    for (int i = 0; i < N; i += 4)
+      asm volatile("ld.relaxed.cluster.shared::cluster.v4.u32 {%0,%1,%2,%3}, [%4];"
+                   : "=r"(r[i]), "=r"(r[i + 1]), "=r"(r[i + 2]), "=r"(r[i + 3]) : "r"(a + 4u * i) : "memory");
+  }
+}
+__device__ __forceinline__ void fence_cluster() { asm volatile("fence.acq_rel.cluster;" ::: "memory"); }
+__device__ __forceinline__ void named_bar_sync(int id, int threads) { asm volatile("bar.sync %0, %1;" :: "r"(id), "r"(threads) : "memory"); }
+__device__ __forceinline__ void nsleep(unsigned ns) { asm volatile("nanosleep.u32 %0;" :: "r"(ns)); }
+__device__ __forceinline__ unsigned long long gtime() { unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+
+// A wait that does not end within two seconds is a scheduling bug: report where and trap, so that the call fails
+// instead of hanging the device.  Compiled in with -DART_WATCHDOG (the test build); free otherwise.
+#ifdef ART_WATCHDOG
+struct Watch {
+  unsigned long long t0; unsigned long long* dbg; int code;
+  __device__ __forceinline__ Watch(unsigned long long* d, int c) : t0(gtime()), dbg(d), code(c) {}
+  __device__ __forceinline__ void poll(int a = 0, int b = 0) {
+    if (gtime() - t0 > 2000000000ull) {
+      if (dbg) { dbg[0] = (static_cast<unsigned long long>(code) << 48) | (static_cast<unsigned long long>(blockIdx.x) << 32) | (static_cast<unsigned>(a) & 0xffffu) << 16 | (static_cast<unsigned>(b) & 0xffffu); __threadfence_system(); }
+      __trap();
+    }
+  }
+};
+#define ART_WATCH(name, code) Watch name(pp.dbg, code)
+#define ART_WATCH_POLL(name, ...) name.poll(__VA_ARGS__)
+#else
+#define ART_WATCH(name, code)
+#define ART_WATCH_POLL(name, ...)
+#endif
+
+// self-validating words: the lowest mantissa bit carries the generation parity of the slot; -inf travels as -1e30
+__device__ __forceinline__ uint32_t tag_word(float v, uint32_t par) { return (__float_as_uint(v) & ~1u) | par; }
+constexpr float kNegBig = -1e30f;
+
+// ----------------------------------------------------------------------------- the kernel
+
+template <int G, int MODE, bool MT = false>
+__global__ void __launch_bounds__(kThreads, (MODE == 2) ? 1 : 2)
+art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK, const __grid_constant__ CUtensorMap tmV) {
+  constexpr bool ART = MODE != 0;
+  constexpr int PW = (MODE == 2) ? kD : 32;
+  constexpr int NP = kPVSlots, NS = kSSlots;
+  constexpr int LBO_P = p_lbo(G), PBUF = p_buf_bytes(G);
+  constexpr bool kTwoPBufs = (G == 8 && MODE == 1);
+  constexpr uint32_t SUMB = sum_bytes(G, PW);
+  constexpr int PF = G * (kD + 2);                       // floats of one partial state
+  using Scan = ChunkScan<G, PW>;
+  const Params& p = pp.b;
+
+  extern __shared__ __align__(1024) uint8_t smem[];
+  const int S = p.stages, NSUM = pp.nsum;
+  const SmemMapP sm = make_smem_map_p(G, PW, S, NSUM, ART);
+  const uint32_t sbase = smem_u32(smem);
+  if ((sbase & 1023u) != 0u) __trap();
+  const uint32_t bars = sbase + sm.bars;
+  auto bar = [&](uint32_t idx) { return bars + idx * 8u; };
+  IterSlot* slots = reinterpret_cast<IterSlot*>(smem + sm.slots);
+  volatile Item* items = reinterpret_cast<volatile Item*>(smem + sm.items);
+  const uint32_t a_misc = sbase + sm.misc;
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int CL = static_cast<int>(cluster_nctarank());
+  const int rank = static_cast<int>(cluster_ctarank());
+  const int cidx = blockIdx.x / CL;
+  const int n_local = (pp.n_groups > cidx) ? (pp.n_groups - cidx + pp.NC - 1) / pp.NC : 0;   // groups cidx, cidx + NC, ...
+  const int n_init = n_local < CL ? n_local : CL;        // opened before the cluster starts: CTA r opens local group r
+
+  // addresses on the cluster's board (rank 0) and in a home CTA
+  auto board_at = [&](int hs, int field) { return mapa(sbase + sm.board + static_cast<uint32_t>(hs) * 32u + field * 4u, 0); };
+  const uint32_t a_next_local = mapa(sbase + sm.board + kHS * 32u, 0);
+  auto hinfo_at = [&](int hs, uint32_t byte_off) { return mapa(sbase + sm.hinfo + static_cast<uint32_t>(hs & 1) * 32u + byte_off, hs >> 1); };
+  enum { B_NEXT = 0, B_T = 1, B_NACT = 2, B_GROUP = 3, B_GEN = 4 };
+  constexpr uint32_t H_DONE = 0, H_GROUP = 8, H_T = 12, H_GEN = 16, H_LOADED = 20, H_JOINED = 24;
+
+  // ---- one-time setup
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 32); }
+    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 1); }
+    for (int s = 0; s < NP; ++s) { mbar_init(bar(sm.pvfull0 + s), 1); mbar_init(bar(sm.pvfree0 + s), 4); }
+    mbar_init(bar(sm.done0), 1); mbar_init(bar(sm.done0 + 1), 1);
+    st_volatile_s32(a_misc + kMOpen, 0); st_volatile_s32(a_misc + kMScanExit, 0); st_volatile_s32(a_misc + kMFlag, 0);
+    for (int s = 0; s < kPVSlots; ++s) st_volatile_s32(a_misc + kMPubCnt + 4u * s, 0);
+    fence_mbar_init();
+  }
+  for (int i = tid; i < kHS; i += kThreads) {
+    reinterpret_cast<int*>(smem + sm.ctrl)[i] = 0;
+    int* e = reinterpret_cast<int*>(smem + sm.board + i * 32);
+    e[B_NEXT] = 0; e[B_T] = 0; e[B_NACT] = 0; e[B_GROUP] = -1; e[B_GEN] = 0;
+  }
+  if (tid == 0) *reinterpret_cast<int*>(smem + sm.board + kHS * 32) = n_init;
+  if (tid < 16) reinterpret_cast<int*>(smem + sm.hinfo)[tid] = 0;
+  if (warp == kWarpMmaPV) tmem_alloc(a_misc + kMTmem, kTmemCols);
+  {
+    if (tid < 64) {                                          // the zero rows behind each Q^T buffer
+      reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + 16 * kQLbo)[tid] = __float2bfloat16_rn(0.f);
+      reinterpret_cast<__nv_bfloat16*>(smem + sm.qb + kQBytes + 16 * kQLbo)[tid] = __float2bfloat16_rn(0.f);
+    }
+    uint4* qz = reinterpret_cast<uint4*>(smem + sm.qb);      // rows >= Gr stay zero for the whole launch
+    for (int idx = tid; idx < 2 * kQBytes / 16; idx += kThreads) qz[idx] = make_uint4(0u, 0u, 0u, 0u);
+    uint4* pz = reinterpret_cast<uint4*>(smem + sm.pb);      // P^T rows are read before they are first written
+    for (int idx = tid; idx < p_bufs(G, S, MODE == 1) * 2 * PBUF / 16; idx += kThreads) pz[idx] = make_uint4(0u, 0u, 0u, 0u);
+  }
+  fence_proxy_async();
+  tc_fence_before();
+  cluster_sync_all();                                        // boards and barriers of every CTA are live
+  tc_fence_after();
+  const uint32_t tmem_base = static_cast<uint32_t>(ld_volatile_s32(a_misc + kMTmem));
+  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kSCols;
+
+  // fold warps: output coordinate and running (un-normalised) partial state of the current visit
+  const int fq = warp & 3;
+  const int d = fq * 32 + lane;
+
+  // decoded progress word of (home slot, generation): last decided step, fired?
+  auto read_ctrl = [&](int hs, int gen, bool& fired) -> int {
+    const int c = ld_ctrl_relaxed(sbase + sm.ctrl + static_cast<uint32_t>(hs) * 4u);
+    if ((static_cast<unsigned>(c) >> 25) != static_cast<unsigned>(gen)) { fired = false; return 0; }
+    fired = (c >> 24) & 1;
+    return c & 0xffffff;
+  };
+
+  // ===================================================== scheduling state of the producer warp (open / join / claim)
+  int it = 0, stage = 0; uint32_t ph = 0;
+  int my_gen = 0;                                          // groups this CTA has opened
+  int nvisit = 0;                                          // visits that issued at least one item
+  int q_last[2] = {-1, -1};                                // last item that reads Q buffer 0 / 1
+  bool more_local = n_local > n_init;
+  // the visit
+  bool have = false;
+  int v_hs = 0, v_gen = 0, v_group = 0, v_T = 0, v_b = 0, v_g = 0, v_L = 0, v_loaded = 0, v_items = 0, v_qsel = 0;
+  Trav v_tr = {};
+
+  auto wait_empty = [&]() {                               // the stage this item will use is free again
+    if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);
+  };
+  auto advance = [&]() { ++it; if (++stage == S) { stage = 0; ph ^= 1u; } };
+  auto push_marker = [&](int kind, int tcode, int meta_extra, unsigned long long payload) {
+    wait_empty();
+    if (lane == 0) {
+      items[it % kItemsRing].tcode = tcode; items[it % kItemsRing].meta = (kind << 6) | meta_extra; items[it % kItemsRing].mask = payload;
+      if (kind == ITEM_END)                               // one END per softmax warp: only the first takes a stage
+        for (int j = 1; j < NS; ++j) { items[(it + j) % kItemsRing].tcode = 0; items[(it + j) % kItemsRing].meta = (ITEM_END << 6); items[(it + j) % kItemsRing].mask = 0ull; }
+      mbar_arrive(bar(sm.full0 + stage));
+    }
+    __syncwarp();
+    advance();
+  };
+  // group -> geometry
+  auto set_group = [&](int group) {
+    v_group = group; v_b = group / p.Hkv; v_g = group % p.Hkv; v_L = p.seq_lens[v_b];
+    v_tr = make_trav(p, v_b, v_g, v_L); v_T = v_tr.T;
+  };
+  // become the home of local group i (lane-uniform); false if the group is empty (handled here)
+  auto open_group = [&](int i) -> bool {
+    set_group(cidx + i * pp.NC);
+    if (v_T == 0) {                                        // no eligible block: out = 0, t* = 0
+      for (int o = lane; o < p.Gr * kD; o += 32) {
+        const int h = o / kD;
+        p.out[((static_cast<int64_t>(v_b) * p.qlen + h / p.Gh) * p.Hq + v_g * p.Gh + h % p.Gh) * kD + (o - h * kD)] = 0.f;
+      }
+      if (lane == 0) p.stop_block[v_group] = 0;
+      return false;
+    }
+    const int hsl = my_gen & 1;
+    v_hs = rank * 2 + hsl; v_gen = my_gen & 127;
+    if (lane == 0) {
+      ART_WATCH(wd, 1);
+      while (atom_cas_cluster_acqrel(board_at(v_hs, B_NACT), 0, kLock) != 0) { nsleep(64); ART_WATCH_POLL(wd, v_hs, my_gen); }
+    }
+    __syncwarp();
+    if constexpr (ART) {                                   // nobody is left who could still write a notice of the slot's last group
+      uint32_t* tg = reinterpret_cast<uint32_t*>(smem + sm.tags) + hsl * kNR;
+      for (int i2 = lane; i2 < kNR; i2 += 32) tg[i2] = 0u;
+    }
+    if (lane == 0) {
+      HomeInfo* hi = reinterpret_cast<HomeInfo*>(smem + sm.hinfo) + hsl;
+      hi->done = ART ? 0ull : (static_cast<unsigned long long>(v_T + 1) << 32);
+      hi->group = v_group; hi->T = v_T; hi->gen = v_gen; hi->loaded = 0; hi->joined = 0u;
+      asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(board_at(v_hs, B_NEXT)), "r"(0) : "memory");
+      asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(board_at(v_hs, B_T)), "r"(v_T) : "memory");
+      asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(board_at(v_hs, B_GROUP)), "r"(v_group) : "memory");
+      asm volatile("st.relaxed.cluster.shared::cluster.s32 [%0], %1;" :: "r"(board_at(v_hs, B_GEN)), "r"(v_gen) : "memory");
+    }
+    __syncwarp();
+    if (lane == 0) {
+      atom_add_cluster_acqrel(board_at(v_hs, B_NACT), 1 - kLock);     // open, one worker (this CTA); releases all of the above
+      if constexpr (ART) asm volatile("st.release.cta.shared::cta.s32 [%0], %1;" :: "r"(a_misc + kMOpen), "r"(my_gen + 1) : "memory");
+    }
+    __syncwarp();
+    ++my_gen;
+    return true;
+  };
+  // the home slot this CTA would open next is free (every worker of the group that used it last has left)
+  auto slot_free = [&]() -> bool {
+    if (my_gen < 2) return true;
+    int v = 0;
+    if (lane == 0) v = ld_cluster_relaxed_s32(board_at(rank * 2 + (my_gen & 1), B_NACT));
+    return __shfl_sync(0xffffffffu, v, 0) == 0;
+  };
+  // join the open group of the cluster with the most unclaimed steps per worker; false if there is none
+  auto join_group = [&]() -> bool {
+    int score = 0, e_next = 0, e_T = 0, e_nact = 0, e_group = -1, e_gen = 0;
+    if (lane < 2 * CL) {
+      e_next = ld_cluster_relaxed_s32(board_at(lane, B_NEXT)); e_T = ld_cluster_relaxed_s32(board_at(lane, B_T));
+      e_nact = ld_cluster_relaxed_s32(board_at(lane, B_NACT)); e_group = ld_cluster_relaxed_s32(board_at(lane, B_GROUP));
+      e_gen = ld_cluster_relaxed_s32(board_at(lane, B_GEN));
+      bool fired = false;
+      if constexpr (ART) read_ctrl(lane, e_gen, fired);
+      const int rem = (e_nact > 0 && e_group >= 0 && !fired) ? e_T - e_next : 0;
+      if (rem >= kMinJoin) score = (rem << 4) / (e_nact + 1) + 1;
+    }
+    int best = score, who = lane;
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) {
+      const int ob = __shfl_xor_sync(0xffffffffu, best, m), ow = __shfl_xor_sync(0xffffffffu, who, m);
+      if (ob > best || (ob == best && ow < who)) { best = ob; who = ow; }
+    }
+    if (best == 0) return false;
+    int ok = 0, T2 = 0, grp = 0, gen2 = 0;
+    if (lane == 0) {
+      const int old = atom_add_cluster_acqrel(board_at(who, B_NACT), 1);        // pin: the slot cannot be reopened under us
+      T2 = ld_cluster_relaxed_s32(board_at(who, B_T)); grp = ld_cluster_relaxed_s32(board_at(who, B_GROUP));
+      gen2 = ld_cluster_relaxed_s32(board_at(who, B_GEN));
+      const int nx = ld_cluster_relaxed_s32(board_at(who, B_NEXT));
+      ok = (old > 0 && grp >= 0 && nx < T2) ? 1 : 0;
+      if (!ok) atom_add_cluster_acqrel(board_at(who, B_NACT), -1);
+    }
+    ok = __shfl_sync(0xffffffffu, ok, 0);
+    if (!ok) return true;                                  // lost a race: look again
+    v_hs = who; v_gen = __shfl_sync(0xffffffffu, gen2, 0);
+    set_group(__shfl_sync(0xffffffffu, grp, 0));
+    have = true;
+    return true;
+  };
+  // leave the current group without having issued an item for it
+  auto leave_quietly = [&]() { if (lane == 0) atom_add_cluster_acqrel(board_at(v_hs, B_NACT), -1); __syncwarp(); };
+
+  if (warp == kWarpProducer && rank < n_init) have = open_group(rank);
+  // every CTA's first group is on the board before anybody looks for a group to join
+  cluster_sync_all();
+
+  if (warp == kWarpProducer) {
+    // ===================================================== A1 + A2: claim steps, resolve blocks, issue TMA loads
+    for (;;) {
+      if (!have) {
+        if (more_local && slot_free()) {
+          int i = 0;
+          if (lane == 0) i = atom_add_cluster(a_next_local, 1);
+          i = __shfl_sync(0xffffffffu, i, 0);
+          if (i < n_local) { have = open_group(i); if (!have) continue; }
+          else more_local = false;
+        }
+        if (!have) {
+          if (!join_group()) {
+            if (!more_local) break;                          // nothing to open, nothing to join: done
+            nsleep(200);                                     // our next slot is still draining
+            continue;
+          }
+          if (!have) continue;
+        }
+        v_loaded = 0; v_items = 0;
+      }
+      // ---- the visit: claim steps until the group has none left (or Algorithm 1 has fired)
+      const uint32_t a_next = board_at(v_hs, B_NEXT), a_nact = board_at(v_hs, B_NACT);
+      auto claim = [&]() -> int { return atom_add_cluster(a_next, 1) + 1; };
+      auto resolve = [&](int t, bool& valid, unsigned long long& mask, int& page, int& ec) {
+        bool fired = false;
+        if constexpr (ART) read_ctrl(v_hs, v_gen, fired);
+        valid = t <= v_T && !fired;
+        mask = 0ull; page = 0; ec = 0;
+        if (valid) {
+          const int blk = trav_block(v_tr, t);
+          mask = block_mask(p, v_L, blk);
+          if constexpr (MT) ec = causal_code(p, v_L, blk);
+          if (mask) page = p.block_table[static_cast<int64_t>(v_b) * p.max_blocks + blk];
+        }
+      };
+      int tB = 0, nactB = 1;
+      if (lane == 0) tB = claim();
+      int tA = __shfl_sync(0xffffffffu, tB, 0);
+      bool validA; unsigned long long maskA; int pageA, ecA;
+      resolve(tA, validA, maskA, pageA, ecA);
+      if (lane == 0 && validA) { tB = claim(); if constexpr (ART) nactB = ld_cluster_relaxed_s32(a_nact); }
+      while (validA) {
+        const int tN = __shfl_sync(0xffffffffu, tB, 0);
+        bool validB; unsigned long long maskB; int pageB, ecB;
+        resolve(tN, validB, maskB, pageB, ecB);
+        if (validB && lane == 0) { tB = claim(); if constexpr (ART) nactB = ld_cluster_relaxed_s32(a_nact); }
+        if constexpr (ART) {
+          // A7 / run-ahead: the loads of step t go out once step t - R is decided (R grows with the workers of the group)
+          int R = pp.rw * max(__shfl_sync(0xffffffffu, nactB, 0), 1);
+          R = R > kNR ? kNR : R;
+          bool fired = false;
+          ART_WATCH(wd, 2);
+          while (read_ctrl(v_hs, v_gen, fired) < tA - R && !fired) { ART_WATCH_POLL(wd, v_hs, tA); }
+          if (fired) break;                                  // t > t*: nothing of this group is loaded any more
+        }
+        if (v_items == 0) {
+          // first item of the visit: this group's Q^T goes into the Q buffer that the visit before last used
+          v_qsel = nvisit & 1;
+          if (q_last[v_qsel] >= 0 && q_last[v_qsel] > it - S) mbar_wait(bar(sm.empty0 + q_last[v_qsel] % S), (q_last[v_qsel] / S) & 1);
+          const __nv_bfloat16* qp = reinterpret_cast<const __nv_bfloat16*>(p.q) + (static_cast<int64_t>(v_b) * p.qlen * p.Hq + v_g * p.Gh) * kD;
+          for (int c = lane; c < p.Gr * (kD / 8); c += 32) {  // 16-byte chunks: row r, columns 8 c8 .. 8 c8 + 7
+            const int row = c / (kD / 8), c8 = c % (kD / 8);
+            const uint4 val = *reinterpret_cast<const uint4*>(qp + ((row / p.Gh) * p.Hq + row % p.Gh) * kD + c8 * 8);
+            *reinterpret_cast<uint4*>(smem + sm.qb + v_qsel * kQBytes + c8 * kQLbo + row * 16) = val;
+          }
+          fence_proxy_async();                               // written by threads, read by the tensor core
+          __syncwarp();
+          ++nvisit;
+        }
+        wait_empty();
+        if (lane == 0) {
+          const uint32_t fb = bar(sm.full0 + stage);
+          const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
+          items[it % kItemsRing].tcode = tA | (ecA << kItemShift);
+          items[it % kItemsRing].meta = v_hs | (v_qsel << 5) | (ITEM_DATA << 6) | (v_gen << 8);
+          items[it % kItemsRing].mask = maskA;
+          if (maskA == 0ull) {
+            mbar_arrive(fb);                                 // nothing to load: an all-masked step
+          } else {
+            int c1, c2;
+            if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = pageA * p.Hkv + v_g; }
+            else { c1 = v_g; c2 = pageA * kBlockTokens; }
+            mbar_arrive_expect_tx(fb, kStageBytes);
+            tma_load_box(dst, &tmK, 0, c1, c2, fb);
+            tma_load_box(dst + kBoxBytes, &tmK, 64, c1, c2, fb);
+            tma_load_box(dst + 2 * kBoxBytes, &tmV, 0, c1, c2, fb);
+            tma_load_box(dst + 3 * kBoxBytes, &tmV, 64, c1, c2, fb);
+          }
+        }
+        __syncwarp();
+        if (maskA != 0ull) ++v_loaded;
+        q_last[v_qsel] = it;
+        ++v_items;
+        advance();
+        tA = tN; validA = validB; maskA = maskB; pageA = pageB; ecA = ecB;
+      }
+      // ---- the group has no step left for us: flush our partial state (the fold warps leave the group for us)
+      if (v_items > 0) push_marker(ITEM_FLUSH, v_loaded, v_hs | (v_gen << 8), static_cast<unsigned long long>(v_group));
+      else leave_quietly();
+      have = false;
+    }
+    push_marker(ITEM_END, 0, 0, 0ull);
+    if (lane == 0) st_volatile_s32(a_misc + kMScanExit, 1);
+  } else if (warp == kWarpMmaS) {
+    // ===================================================== A3: S = K_t Q^T, rows = tokens, columns = heads
+    if (lane == 0) {
+      const uint64_t dK = kDescSw128 | desc_strides(16, 1024);
+      const uint64_t dQ = kDescNoSw | desc_strides(kQLbo, kQSbo);
+      int st = 0; uint32_t ph = 0;
+      for (int i = 0;; ++i) {
+        const int q = i & (NS - 1);
+        mbar_wait(bar(sm.full0 + st), ph);
+        const int meta = items[i % kItemsRing].meta;
+        const int kind = item_kind(meta);
+        if (kind == ITEM_END) {                              // wake every softmax warp once more; each finds its END item
+          for (int j = 0; j < NS; ++j) {
+            const int ii = i + j, qq = ii & (NS - 1);
+            if (ii >= NS) mbar_wait(bar(sm.sfree0 + qq), ((ii / NS) - 1) & 1);
+            umma_commit(bar(sm.sfull0 + qq));
+          }
+          break;
+        }
+        if (i >= NS) mbar_wait(bar(sm.sfree0 + q), ((i / NS) - 1) & 1);
+        if (kind == ITEM_DATA) {
+          tc_fence_after();
+          const uint32_t qb = sbase + sm.qb + item_q(meta) * kQBytes;
+          const uint32_t kt = sbase + sm.ring + st * kStageBytes - q * 4096;
+          const uint32_t dcol = tmem_S + q * kSCols;
+#pragma unroll
+          for (int ks = 0; ks < 8; ++ks) {
+            const uint32_t ka = kt + (ks >> 2) * kBoxBytes + (ks & 3) * 32;
+            const uint64_t bq = dQ | desc_addr(qb + ks * 2 * kQLbo);
+            umma_bf16(dcol, dK | desc_addr(ka), bq, kIdescS, ks > 0);
+            umma_bf16(dcol + kUmmaN, dK | desc_addr(ka + 4096), bq, kIdescS, ks > 0);
+          }
+        }
+        umma_commit(bar(sm.sfull0 + q));
+        if (++st == S) { st = 0; ph ^= 1u; }
+      }
+      umma_commit(bar(sm.done0));
+      mbar_wait(bar(sm.done0), 0);
+    }
+  } else if (warp == kWarpMmaPV) {
+    // ===================================================== A5: P~V_t = V_t^T P^T, rows = d, columns = heads
+    if (lane == 0) {
+      const uint64_t dV = kDescSw128 | desc_strides(kBoxBytes, 1024);
+      const uint64_t dP = kDescNoSw | desc_strides(LBO_P, 128);
+      int st = 0; uint32_t ph = 0;
+      for (int i = 0;; ++i) {
+        const int ps = i & (NP - 1);
+        mbar_wait(bar(sm.pfull0 + st), ph);
+        const int kind = item_kind(items[i % kItemsRing].meta);
+        if (i >= NP) mbar_wait(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1);
+        if (kind == ITEM_DATA) {
+          tc_fence_after();
+          const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
+          const uint32_t pb = sbase + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF;
+#pragma unroll
+          for (int part = 0; part < 2; ++part)
+#pragma unroll
+            for (int ks = 0; ks < 4; ++ks)
+              umma_bf16(tmem_PV + ps * kUmmaN, dV | desc_addr(vt + ks * 2048),
+                        dP | desc_addr(pb + part * PBUF + ks * 2 * LBO_P), kIdescPV, (part | ks) > 0);
+        }
+        umma_commit(bar(sm.empty0 + st));
+        umma_commit(bar(sm.pvfull0 + ps));
+        if (kind == ITEM_END) break;
+        if (++st == S) { st = 0; ph ^= 1u; }
+      }
+      umma_commit(bar(sm.done0 + 1));
+      mbar_wait(bar(sm.done0 + 1), 0);
+    }
+  } else if (warp >= kWarpSoftmax0 && warp < kWarpSoftmax0 + 4) {
+    // ===================================================== A4: block-local softmax, two tokens per thread
+    const int q = warp - kWarpSoftmax0;
+    const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
+    int st = q % S;
+    for (int i = q;; i += NS) {
+      mbar_wait(bar(sm.sfull0 + q), (i / NS) & 1);
+      const int kind = item_kind(items[i % kItemsRing].meta);
+      if (kind == ITEM_END) {
+        // the END item that owns a stage is the first of the four; only its warp hands it on to the P.V issuer
+        if (item_kind(items[(i + kItemsRing - 1) % kItemsRing].meta) != ITEM_END || i == 0) mbar_arrive(bar(sm.pfull0 + st));
+        break;
+      }
+      if (kind != ITEM_DATA) {                               // a marker: nothing to compute
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+        mbar_arrive(bar(sm.pfull0 + st));
+        st += NS; while (st >= S) st -= S;
+        continue;
+      }
+      tc_fence_after();
+      float s0[G], s1[G];
+      tmem_ld<G>(taddr, s0);
+      tmem_ld<G>(taddr + kUmmaN, s1);
+      tmem_ld_wait();
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+      if (kTwoPBufs && i >= 2) mbar_wait(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1);
+      const unsigned long long vmask = items[i % kItemsRing].mask;
+      const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
+      float mb[G];
+      int ec = 0;
+      if constexpr (MT) ec = items[i % kItemsRing].tcode >> kItemShift;
+      if (MT && ec != 0) {                                    // R15: the most recent tokens are cut row by row
+#pragma unroll
+        for (int h = 0; h < G; ++h) {
+          const int lim = ec - static_cast<int>((p.cuts >> (4 * h)) & 15u);
+          s0[h] = (v0 && lane < lim) ? s0[h] * p.scale_log2 : kNegInf;
+          s1[h] = (v1 && lane + 32 < lim) ? s1[h] * p.scale_log2 : kNegInf;
+          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
+        }
+      } else {
+#pragma unroll
+        for (int h = 0; h < G; ++h) {
+          s0[h] = v0 ? s0[h] * p.scale_log2 : kNegInf;        // masked tokens: weight 0 (R8); their K may be NaN
+          s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
+          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
+        }
+      }
+      uint8_t* pb0 = smem + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;
+      float ls[G];
+#pragma unroll
+      for (int h = 0; h < G; ++h) {
+        const float p0 = (v0 && mb[h] != kNegInf) ? fast_exp2(s0[h] - mb[h]) : 0.f;
+        const float p1 = (v1 && mb[h] != kNegInf) ? fast_exp2(s1[h] - mb[h]) : 0.f;
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(p0), h1 = __float2bfloat16_rn(p1);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(p0 - __bfloat162float(h0)), l1 = __float2bfloat16_rn(p1 - __bfloat162float(h1));
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16) = h0;
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + 4 * LBO_P) = h1;
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF) = l0;
+        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF + 4 * LBO_P) = l1;
+        ls[h] = (__bfloat162float(h0) + __bfloat162float(l0)) + (__bfloat162float(h1) + __bfloat162float(l1));
+      }
+      if (vmask != ~0ull) {                                   // masked V rows may hold NaN: 0 * NaN would poison P~V
+        uint4* vr = reinterpret_cast<uint4*>(smem + sm.ring + st * kStageBytes + 2 * kBoxBytes);
+        if (!v0) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) { vr[lane * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[lane * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
+        }
+        if (!v1) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) { vr[(lane + 32) * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[(lane + 32) * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
+        }
+      }
+      Reduce32<G, 16>::run(ls, lane);
+      {
+        const int hh = head_of_lane32<G>(lane);
+        float mine = mb[0];
+#pragma unroll
+        for (int h = 1; h < G; ++h) mine = (hh == h) ? mb[h] : mine;
+        IterSlot& slot = slots[i & (kIterSlots - 1)];
+        if ((lane & (32 / G - 1)) == 0) { slot.mref[hh] = mine; slot.lsum[hh] = ls[0]; }
+      }
+      fence_proxy_async();
+      mbar_arrive(bar(sm.pfull0 + st));
+      st += NS; while (st >= S) st -= S;
+    }
+  } else if (warp < kWarpFold0 + 4) {
+    // ===================================================== A5 / A6 / A8 / A9: publish summaries, merge P~V_t, flush, combine
+    const uint32_t tlane = static_cast<uint32_t>(fq * 32) << 16;
+    float acc[G], m_tot[G], l_tot[G];
+    int nfold = 0;
+    auto reset_state = [&]() {
+#pragma unroll
+      for (int h = 0; h < G; ++h) { acc[h] = 0.f; m_tot[h] = kNegInf; l_tot[h] = 0.f; }
+      nfold = 0;
+    };
+    reset_state();
+    auto release_pv = [&](int i) {
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(sm.pvfree0 + (i & (NP - 1))));
+    };
+    auto fold = [&](int i) {
+      tc_fence_after();
+      float pv[G];
+      tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN, pv);
+      tmem_ld_wait();
+      const IterSlot& sl = slots[i & (kIterSlots - 1)];
+#pragma unroll
+      for (int h = 0; h < G; ++h) {
+        const float mr = sl.mref[h];
+        if (mr != kNegInf) {                                  // a block with no valid token changes nothing
+          const float mn = fmaxf(m_tot[h], mr);
+          const float a = fast_exp2(m_tot[h] - mn), bb = fast_exp2(mr - mn);
+          acc[h] = fmaf(a, acc[h], bb * pv[h]);
+          l_tot[h] = fmaf(a, l_tot[h], bb * sl.lsum[h]);
+          m_tot[h] = mn;
+        }
+      }
+      ++nfold;
+      release_pv(i);
+    };
+    // out[row h] = combination of the partial states of the CTAs in `joined` (flash-decoding merge)
+    auto combine = [&](int group, unsigned joined, int T) {
+      const int b = group / p.Hkv, g = group % p.Hkv;
+      const bool alone = joined == (1u << rank);
+#pragma unroll
+      for (int h = 0; h < G; ++h) {
+        float a = acc[h], l = l_tot[h];
+        if (!alone) {
+          float mx = kNegInf;
+          for (unsigned js = joined; js; js &= js - 1) {
+            const int c = __ffs(js) - 1;
+            mx = fmaxf(mx, __ldcg(pp.part + (static_cast<size_t>(group) * CL + c) * PF + G * kD + h));
+          }
+          a = 0.f; l = 0.f;
+          for (unsigned js = joined; js; js &= js - 1) {
+            const int c = __ffs(js) - 1;
+            const float* pc = pp.part + (static_cast<size_t>(group) * CL + c) * PF;
+            const float mc = __ldcg(pc + G * kD + h);
+            const float f = (mc == kNegInf) ? 0.f : fast_exp2(mc - mx);
+            a = fmaf(f, __ldcg(pc + h * kD + d), a);
+            l = fmaf(f, __ldcg(pc + G * kD + G + h), l);
+          }
+        }
+        if (h < p.Gr)                                         // Alg. 1 l.18; row h = query token h / Gh, head h % Gh
+          p.out[((static_cast<int64_t>(b) * p.qlen + h / p.Gh) * p.Hq + g * p.Gh + h % p.Gh) * kD + d] = (l > 0.f) ? a / l : 0.f;
+      }
+      if (!ART && d == 0) p.stop_block[group] = T;
+    };
+    // end of a visit: hand the partial state over, combine if we are the last, leave the group
+    auto flush = [&](int tcode, int meta, unsigned long long payload) {
+      const int hs = item_hs(meta), group = static_cast<int>(payload);
+      if (nfold > 0) {
+        float* part = pp.part + (static_cast<size_t>(group) * CL + rank) * PF;
+#pragma unroll
+        for (int h = 0; h < G; ++h) {
+          part[h * kD + d] = acc[h];
+          if (d == 0) { part[G * kD + h] = m_tot[h]; part[G * kD + G + h] = l_tot[h]; }
+        }
+        __threadfence();
+      }
+      named_bar_sync(1, 128);
+      if (warp == kWarpFold0 && lane == 0) {
+        int flag = 0;
+        if (p.blocks_loaded && tcode > 0) atomicAdd(p.blocks_loaded + group, tcode);
+        if (nfold > 0) {
+          atom_or_cluster(hinfo_at(hs, H_JOINED), 1u << rank);
+          const unsigned long long old = atom_add64_cluster_acqrel(hinfo_at(hs, H_DONE), static_cast<unsigned long long>(nfold));
+          const unsigned long long tot = old + static_cast<unsigned long long>(nfold);
+          const unsigned hi = static_cast<unsigned>(tot >> 32), lo = static_cast<unsigned>(tot);
+          if (hi != 0u && lo == hi - 1u) {                    // every step <= t* is folded and flushed: we combine
+            flag = static_cast<int>(hi);
+            st_volatile_s32(a_misc + kMJoined, static_cast<int>(ld_cluster_u32(hinfo_at(hs, H_JOINED))));
+          }
+        }
+        st_volatile_s32(a_misc + kMFlag, flag);
+      }
+      named_bar_sync(1, 128);
+      const int flag = ld_volatile_s32(a_misc + kMFlag);
+      if (flag) {
+        __threadfence();
+        combine(group, static_cast<unsigned>(ld_volatile_s32(a_misc + kMJoined)), flag - 1);
+      }
+      named_bar_sync(1, 128);                                 // the flag is read by all before the next flush rewrites it
+      if (warp == kWarpFold0 && lane == 0) atom_add_cluster_acqrel(board_at(hs, B_NACT), -1);   // leave (after everything above)
+      reset_state();
+    };
+
+    if constexpr (!ART) {
+      for (int i = 0;; ++i) {
+        mbar_wait(bar(sm.pvfull0 + (i & (NP - 1))), (i / NP) & 1);
+        const int meta = items[i % kItemsRing].meta;
+        const int kind = item_kind(meta);
+        if (kind == ITEM_DATA) { fold(i); continue; }
+        if (kind == ITEM_END) break;
+        flush(items[i % kItemsRing].tcode, meta, items[i % kItemsRing].mask);
+        release_pv(i);
+      }
+    } else {
+      int pub = 0, fld = 0;
+      bool pub_ready = false;
+      ART_WATCH(wd, 3);
+      for (;;) {
+        // ---- the oldest unfolded item: merge it once its step is decided, drop it if it lies beyond t*
+        if (fld < pub) {
+          const int meta = items[fld % kItemsRing].meta;
+          const int kind = item_kind(meta);
+          if (kind == ITEM_DATA) {
+            bool fired;
+            const int tdec = read_ctrl(item_hs(meta), item_gen(meta), fired);
+            const int tf = items[fld % kItemsRing].tcode & kItemStep;
+            if (fired && tf > tdec) { release_pv(fld); ++fld; continue; }
+            if (tdec >= tf) { fold(fld); ++fld; continue; }   // decided: the scan has read this step's summary
+          } else if (kind == ITEM_FLUSH) {
+            flush(items[fld % kItemsRing].tcode, meta, items[fld % kItemsRing].mask);
+            release_pv(fld); ++fld; continue;
+          } else {
+            break;                                            // END
+          }
+        }
+        // ---- the next finished item: write its summary, tell the group's home where it is
+        if (pub - fld < NSUM) {
+          const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
+          const uint32_t par = (pub / NP) & 1;
+          if (!pub_ready) pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
+          if (pub_ready) {
+            const int meta = items[pub % kItemsRing].meta;
+            if (item_kind(meta) == ITEM_DATA) {
+              const int hs = item_hs(meta), t = items[pub % kItemsRing].tcode & kItemStep;
+              const int sslot = pub % NSUM;
+              const uint32_t gpar = static_cast<uint32_t>(pub / NSUM) & 1u;
+              tc_fence_after();
+              float pv[G];
+              tmem_ld<G>(tmem_PV + tlane + (pub & (NP - 1)) * kUmmaN, pv);
+              tmem_ld_wait();
+              uint32_t* sw = reinterpret_cast<uint32_t*>(smem + sm.sums + sslot * SUMB);
+              if (MODE == 2 || (d & 3) == 0) {
+                const int pi = (MODE == 2) ? d : (d >> 2);    // probe coordinate k * (d / 32)  (R1)
+                const int sub = pi % Scan::LPH, j = pi / Scan::LPH;
+#pragma unroll
+                for (int h = 0; h < G; ++h) sw[(h * Scan::LPH + sub) * Scan::CPL + j] = tag_word(pv[h], gpar);
+              }
+              if (d == 1) {
+                const IterSlot& sl = slots[pub & (kIterSlots - 1)];
+#pragma unroll
+                for (int h = 0; h < G; ++h) {
+                  sw[G * PW + 2 * h] = tag_word(fmaxf(sl.mref[h], kNegBig), gpar);
+                  sw[G * PW + 2 * h + 1] = tag_word(sl.lsum[h], gpar);
+                }
+              }
+              __syncwarp();
+              // the notice: step number, producing CTA, slot, parity; sent by the warp that finishes last
+              if (lane == 0) {
+                const int prev = atomicAdd(reinterpret_cast<int*>(smem + sm.misc + kMPubCnt) + sslot, 1);
+                if ((prev & 3) == 3) {
+                  const uint32_t word = (static_cast<uint32_t>(t) << 8) | (static_cast<uint32_t>(rank) << 4) | (gpar << 3) | static_cast<uint32_t>(sslot);
+                  const uint32_t dst = mapa(sbase + sm.tags + (static_cast<uint32_t>(hs & 1) * kNR + static_cast<uint32_t>((t - 1) % kNR)) * 4u, hs >> 1);
+                  asm volatile("st.relaxed.cluster.shared::cluster.u32 [%0], %1;" :: "r"(dst), "r"(word) : "memory");
+                }
+              }
+            }
+            ++pub; pub_ready = false;
+            continue;
+          }
+        }
+        ART_WATCH_POLL(wd, fld, pub);
+      }
+    }
+  } else if (ART && warp == kWarpScan) {
+    // ===================================================== A6 + A7 + A9: Algorithm 1 over step summaries (home of a group)
+    constexpr int LPH = Scan::LPH, CPL = Scan::CPL, NBK = Scan::NBK, STRIDE = Scan::STRIDE;
+    const int sub = lane % LPH;
+    const bool owner = (sub % STRIDE) == 0;
+    const int own_k = sub / STRIDE;                          // the step of a chunk this lane owns for its head
+    const int h_lane = lane / LPH;
+    int sg = 0;
+    for (;;) {
+      {
+        ART_WATCH(wd, 4);
+        bool stop = false;
+        for (;;) {
+          int oc;
+          asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(oc) : "r"(a_misc + kMOpen) : "memory");
+          if (oc > sg) break;
+          if (ld_volatile_s32(a_misc + kMScanExit)) {
+            asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(oc) : "r"(a_misc + kMOpen) : "memory");
+            if (oc > sg) break;
+            stop = true; break;
+          }
+          nsleep(100);
+          ART_WATCH_POLL(wd, sg, 0);
+        }
+        if (stop) break;
+      }
+      const int hsl = sg & 1, hs = rank * 2 + hsl;
+      const HomeInfo* hi = reinterpret_cast<const HomeInfo*>(smem + sm.hinfo) + hsl;
+      const int group = *reinterpret_cast<const volatile int*>(&hi->group), Tn = *reinterpret_cast<const volatile int*>(&hi->T);
+      const int gen = *reinterpret_cast<const volatile int*>(&hi->gen);
+      const uint32_t tg = sbase + sm.tags + static_cast<uint32_t>(hsl) * kNR * 4u;
+      Scan sc; sc.init(p.Gr);
+      int t = 1, t_stop = 0;
+      while (t <= Tn) {
+        // ---- which of the next NBK steps have arrived (lane k looks at step t + k)
+        uint32_t word = 0u;
+        int n;
+        {
+          ART_WATCH(wd, 5);
+          for (;;) {
+            bool ok = false;
+            if (lane < NBK && t + lane <= Tn) {
+              word = static_cast<uint32_t>(ld_volatile_s32(tg + static_cast<uint32_t>((t + lane - 1) % kNR) * 4u));
+              ok = (word >> 8) == static_cast<uint32_t>(t + lane);
+            }
+            const uint32_t bits = __ballot_sync(0xffffffffu, ok);
+            n = __ffs(~bits) - 1;
+            if (n > 0) break;
+            ART_WATCH_POLL(wd, hs, t);
+          }
+        }
+        // ---- pull the summaries: (m, l) of the owned step, P~V_t of every step at this lane's coordinates
+        float pv[NBK][CPL];
+        float m_own, l_own;
+        {
+          ART_WATCH(wd, 6);
+          for (;;) {
+            bool bad = false;
+            const uint32_t wk_own = __shfl_sync(0xffffffffu, word, own_k);
+            m_own = kNegInf; l_own = 0.f;
+            if (owner && own_k < n) {
+              const uint32_t base = mapa(sbase + sm.sums + (wk_own & 7u) * SUMB, (wk_own >> 4) & 15u);
+              uint32_t ml[2];
+              ld_cluster_vec<2>(base + (G * PW + 2 * h_lane) * 4u, ml);
+              const uint32_t par = (wk_own >> 3) & 1u;
+              bad = ((ml[0] ^ par) | (ml[1] ^ par)) & 1u;
+              m_own = __uint_as_float(ml[0]); l_own = __uint_as_float(ml[1]);
+              if (m_own <= -1e29f) m_own = kNegInf;
+            }
+#pragma unroll
+            for (int k = 0; k < NBK; ++k) {
+              const uint32_t wk = __shfl_sync(0xffffffffu, word, k);
+              if (k < n) {
+                const uint32_t base = mapa(sbase + sm.sums + (wk & 7u) * SUMB, (wk >> 4) & 15u);
+                uint32_t raw[CPL];
+                ld_cluster_vec<CPL>(base + static_cast<uint32_t>(lane * CPL) * 4u, raw);
+                const uint32_t par = (wk >> 3) & 1u;
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) { bad |= ((raw[j] ^ par) & 1u) != 0u; pv[k][j] = __uint_as_float(raw[j]); }
+              } else {
+#pragma unroll
+                for (int j = 0; j < CPL; ++j) pv[k][j] = 0.f;
+              }
+            }
+            if (!__any_sync(0xffffffffu, bad)) break;         // a word of the slot's previous generation: look again
+            ART_WATCH_POLL(wd, hs, t);
+          }
+        }
+        const int fired = sc.chunk(n, lane, p.tau, p.phi, p.patience, m_own, l_own, pv);
+        const int t_last = fired >= 0 ? t + fired : t + n - 1;
+        const bool fin = fired >= 0 || t_last >= Tn;
+        if (fin) {
+          // t* is known: record it, let the last flusher recognise itself, THEN release the final progress word
+          t_stop = t_last;
+          if (lane == 0) {
+            p.stop_block[group] = t_stop;                    // t* (R9)
+            atom_add64_cluster_acqrel(hinfo_at(hs, H_DONE), static_cast<unsigned long long>(t_stop + 1) << 32);
+          }
+          __syncwarp();
+          if (lane < CL) st_cluster_release_s32(mapa(sbase + sm.ctrl + static_cast<uint32_t>(hs) * 4u, lane), ctrl_word(gen, fired >= 0, t_last));
+          break;
+        }
+        if (lane < CL) st_cluster_relaxed_s32(mapa(sbase + sm.ctrl + static_cast<uint32_t>(hs) * 4u, lane), ctrl_word(gen, false, t_last));
+        t += n;
+      }
+      (void)t_stop;
+      ++sg;
+    }
+  }
+
+  // ===================================================== every role is done; peers may still read our shared memory
+  tc_fence_before();
+  __syncthreads();
+  cluster_sync_all();
+  if (warp == kWarpMmaPV) { tc_fence_after(); tmem_dealloc(tmem_base, kTmemCols); }
+}
+
+}  // namespace pc
+}  // namespace art

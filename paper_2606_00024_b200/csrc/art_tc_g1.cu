@@ -1,0 +1,3 @@
+// art_decode_tc_kernel<G = 1, MODE, MT>: instantiations and launcher (see art_launch.h)
+#define ART_TC_G 1
+#include "art_tc_inst.inc"

@@ -66,13 +66,13 @@ def test_argument_validation_happens_before_cuda(art):
     assert _call_off(art, good_desc(art, policy=1, sink_tokens=-1)) == -2
     assert _call_off(art, good_desc(art, split=17)) == -2                    # cluster size > 16
     assert _call_off(art, good_desc(art, split=-2)) == -2
+    assert _call_off(art, good_desc(art, max_blocks_per_seq=1 << 24)) == -2   # a step number is 24 bits
     assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=-1)) == -3   # dynamic: bf16 only
     assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=3)) == -2   # fp32 path: power of two
     assert _call_off(art, good_desc(art), k=33) == -4                        # ART_ERR_ALIGN
     # multi-token queries (q_len, reading R15): m * G <= 8, a cluster schedule
     assert _call_off(art, good_desc(art, q_len=3)) == -2                     # 3 * 4 rows
     assert _call_off(art, good_desc(art, q_len=-1)) == -2
-    assert _call_off(art, good_desc(art, q_len=2, split=-1)) == -2           # not with the dynamic scheduler
     assert _call_off(art, good_desc(art, q_len=3, dtype=art.ART_DTYPE_F32, head_dim=64, num_q_heads=6)) == -2   # 3 * 3 rows
     lib = art.load_library()
     th = art.ArtThresholds(tau=1e-5, phi=1e-3, patience=0, probe_dim=32)
