@@ -281,24 +281,44 @@ static int choose_pc(int G, int mode, int want, int groups, const PcPlan& pl, in
 
 // run-ahead per worker of the persistent-cluster kernel (steps whose loads may be issued beyond the last decided
 // step, per CTA working on the group); ART_PC_RUNAHEAD overrides it for measurements
+static int pc_claim() {
+  static const int env = [] { const char* e = getenv("ART_PC_CLAIM"); return e ? atoi(e) : 0; }();
+  return env > 0 ? (env > 16 ? 16 : env) : 4;
+}
+static unsigned pc_nap() {
+  static const int env = [] { const char* e = getenv("ART_PC_NAP"); return e ? atoi(e) : -1; }();
+  return env >= 0 ? static_cast<unsigned>(env) : 100u;
+}
 static int pc_run_ahead(int nsum) {
   static const int env = [] { const char* e = getenv("ART_PC_RUNAHEAD"); return e ? atoi(e) : 0; }();
   int rw = env > 0 ? env : 6;
   return rw;
 }
 
-#ifdef ART_WATCHDOG
+#if defined(ART_WATCHDOG) || defined(ART_PC_STATS)
 // debugging build: a pinned, device-mapped word that a wait which never ends writes before it traps; it survives
 // the death of the context, so the test harness can print where the kernel was stuck (art_debug_watchdog())
 static unsigned long long* g_watchdog_host = nullptr;
 static unsigned long long* watchdog_word() {
   static unsigned long long* dev = [] {
     unsigned long long* h = nullptr; unsigned long long* dptr = nullptr;
-    if (cudaHostAlloc(&h, 64, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return dptr; }
-    h[0] = 0ull;
+    if (cudaHostAlloc(&h, 512, cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); return dptr; }
+    for (int i = 0; i < 64; ++i) h[i] = 0ull;
     if (cudaHostGetDevicePointer(&dptr, h, 0) != cudaSuccess) { cudaGetLastError(); return static_cast<unsigned long long*>(nullptr); }
     g_watchdog_host = h;
     return dptr;
+  }();
+  return dev;
+}
+#endif
+
+#ifdef ART_PC_STATS
+static unsigned long long* stats_buffer() {
+  static unsigned long long* dev = [] {
+    unsigned long long* d = nullptr;
+    if (cudaMalloc(&d, 512) != cudaSuccess) { cudaGetLastError(); return static_cast<unsigned long long*>(nullptr); }
+    cudaMemset(d, 0, 512);
+    return d;
   }();
   return dev;
 }
@@ -355,10 +375,13 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
     p.stages = pl.stages; p.mbox_slots = 0; p.dyn = 1;
     pc::PcParams pp = {};
     pp.b = p; pp.n_groups = groups; pp.NC = NC; pp.part = static_cast<float*>(workspace);
-    pp.rw = pc_run_ahead(pl.nsum); pp.nsum = pl.nsum > 0 ? pl.nsum : 1;
+    pp.rw = pc_run_ahead(pl.nsum); pp.claim = mode != 0 ? 1 : pc_claim(); pp.nap = pc_nap(); pp.nsum = pl.nsum > 0 ? pl.nsum : 1;
     pp.dbg = nullptr;
-#ifdef ART_WATCHDOG
+#if defined(ART_WATCHDOG) || defined(ART_PC_STATS)
     pp.dbg = watchdog_word();
+#endif
+#ifdef ART_PC_STATS
+    pp.stats = stats_buffer();
 #endif
     CUtensorMap tmK, tmV;
     if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
@@ -661,8 +684,18 @@ const char* art_status_string(int status) {
 
 int art_version(void) { return ART_VERSION; }
 
-#ifdef ART_WATCHDOG
+#if defined(ART_WATCHDOG) || defined(ART_PC_STATS)
 unsigned long long art_debug_watchdog(void) { return art::g_watchdog_host ? art::g_watchdog_host[0] : 0ull; }
+unsigned long long art_debug_watchdog2(void) { return art::g_watchdog_host ? art::g_watchdog_host[1] : 0ull; }
+#ifdef ART_PC_STATS
+void art_debug_stats_read(unsigned long long* host_out) {      // synchronises; returns and clears the 64 counters
+  unsigned long long* d = art::stats_buffer();
+  if (!d) return;
+  cudaDeviceSynchronize();
+  cudaMemcpy(host_out, d, 512, cudaMemcpyDeviceToHost);
+  cudaMemset(d, 0, 512);
+}
+#endif
 #endif
 
 }  // extern "C"

@@ -48,7 +48,10 @@ struct PcParams {
   float* part;                               // workspace: partial states [group][rank][G * (kD + 2)]
   int32_t rw;                                // run-ahead per worker (steps issued beyond the last decided one)
   int32_t nsum;                              // summary slots per CTA (<= kPVSlots)
+  int32_t claim;                             // steps claimed per atomic (a chunk of consecutive steps)
+  uint32_t nap;                              // nanoseconds a polling warp sleeps between two looks
   unsigned long long* dbg;                   // ART_WATCHDOG: where a wait that never ended reports itself
+  unsigned long long* stats;                 // ART_PC_STATS: cycle counters (device memory)
 };
 
 enum { ITEM_DATA = 0, ITEM_FLUSH = 1, ITEM_END = 2 };
@@ -66,7 +69,7 @@ struct BoardEntry { int next, T, nact, group, gen, pad0, pad1, pad2; };        /
 struct HomeInfo { unsigned long long done; int group, T, gen, loaded; unsigned joined; int pad; };   // home CTA: one per local slot
 
 struct SmemMapP {
-  uint32_t qb, pb, slots, items, sums, tags, hinfo, ctrl, board, bars, misc, ring, total;
+  uint32_t qb, pb, slots, items, sums, tags, stab, hinfo, ctrl, board, bars, misc, ring, total;
   uint32_t full0, empty0, pfull0, sfull0, sfree0, pvfull0, pvfree0, done0, nbars;
 };
 // summary of one step: [G * PW] probe values (lane l of the scan warp owns floats l*CPL .. l*CPL + CPL - 1), then (m, l) x G
@@ -77,11 +80,12 @@ __host__ __device__ inline SmemMapP make_smem_map_p(int G, int PW, int stages, i
   uint32_t off = 0;
   m.qb = off; off += 2u * kQBytes;
   m.pb = off; off += static_cast<uint32_t>(p_bufs(G, stages, art && PW == 32)) * 2u * p_buf_bytes(G);
-  m.slots = off; off += kIterSlots * static_cast<uint32_t>(sizeof(IterSlot));
+  m.slots = off; off += kIterSlots * static_cast<uint32_t>(2 * G) * 4u;           // per item: m_blk[G], block sum[G]
   m.items = off; off += kItemsRing * static_cast<uint32_t>(sizeof(Item));
   off = (off + 15u) & ~15u;
   m.sums = off; off += art ? static_cast<uint32_t>(nsum) * sum_bytes(G, PW) : 0u;
   m.tags = off; off += art ? 2u * kNR * 4u : 0u;
+  m.stab = off; off += art ? 2u * 4u * kNR : 0u;                 // per-step results of the four scanning warps
   off = (off + 15u) & ~15u;
   m.hinfo = off; off += 2u * static_cast<uint32_t>(sizeof(HomeInfo));
   m.ctrl = off; off += kHS * 4u;
@@ -108,11 +112,16 @@ constexpr uint32_t kMTmem = 0, kMOpen = 4, kMScanExit = 8, kMFlag = 12, kMJoined
 __device__ __forceinline__ int atom_add_cluster(uint32_t a, int v) {           // relaxed
   int r; asm volatile("atom.relaxed.cluster.shared::cluster.add.s32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
 }
-__device__ __forceinline__ int atom_add_cluster_acqrel(uint32_t a, int v) {
-  int r; asm volatile("atom.acq_rel.cluster.shared::cluster.add.s32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
+// release = MEMBAR.ALL.GPU + atom (about a microsecond under load); acquire = atom + CCTL.IVALL (cheap): every
+// atomic below carries exactly the ordering its use needs
+__device__ __forceinline__ int atom_add_cluster_acquire(uint32_t a, int v) {
+  int r; asm volatile("atom.acquire.cluster.shared::cluster.add.s32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
 }
-__device__ __forceinline__ int atom_cas_cluster_acqrel(uint32_t a, int cmp, int v) {
-  int r; asm volatile("atom.acq_rel.cluster.shared::cluster.cas.b32 %0, [%1], %2, %3;" : "=r"(r) : "r"(a), "r"(cmp), "r"(v) : "memory"); return r;
+__device__ __forceinline__ int atom_add_cluster_release(uint32_t a, int v) {
+  int r; asm volatile("atom.release.cluster.shared::cluster.add.s32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
+}
+__device__ __forceinline__ int atom_cas_cluster_acquire(uint32_t a, int cmp, int v) {
+  int r; asm volatile("atom.acquire.cluster.shared::cluster.cas.b32 %0, [%1], %2, %3;" : "=r"(r) : "r"(a), "r"(cmp), "r"(v) : "memory"); return r;
 }
 __device__ __forceinline__ unsigned atom_or_cluster(uint32_t a, unsigned v) {
   unsigned r; asm volatile("atom.relaxed.cluster.shared::cluster.or.b32 %0, [%1], %2;" : "=r"(r) : "r"(a), "r"(v) : "memory"); return r;
@@ -132,14 +141,14 @@ __device__ __forceinline__ uint32_t ld_cluster_u32(uint32_t a) {
 }
 template <int N> __device__ __forceinline__ void ld_cluster_vec(uint32_t a, uint32_t (&r)[N]) {
   if constexpr (N == 1) {
-    asm volatile("ld.relaxed.cluster.shared::cluster.u32 %0, [%1];" : "=r"(r[0]) : "r"(a) : "memory");
+    asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(r[0]) : "r"(a) : "memory");
   } else if constexpr (N == 2) {
-    asm volatile("ld.relaxed.cluster.shared::cluster.v2.u32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(a) : "memory");
+    asm volatile("ld.shared::cluster.v2.u32 {%0,%1}, [%2];" : "=r"(r[0]), "=r"(r[1]) : "r"(a) : "memory");
   } else {
     static_assert(N % 4 == 0, "vector width");
 #pragma unroll
     for (int i = 0; i < N; i += 4)
-      asm volatile("ld.relaxed.cluster.shared::cluster.v4.u32 {%0,%1,%2,%3}, [%4];"
+      asm volatile("ld.shared::cluster.v4.u32 {%0,%1,%2,%3}, [%4];"
                    : "=r"(r[i]), "=r"(r[i + 1]), "=r"(r[i + 2]), "=r"(r[i + 3]) : "r"(a + 4u * i) : "memory");
   }
 }
@@ -155,8 +164,8 @@ struct Watch {
   unsigned long long t0; unsigned long long* dbg; int code;
   __device__ __forceinline__ Watch(unsigned long long* d, int c) : t0(gtime()), dbg(d), code(c) {}
   __device__ __forceinline__ void poll(int a = 0, int b = 0) {
-    if (gtime() - t0 > 2000000000ull) {
-      if (dbg) { dbg[0] = (static_cast<unsigned long long>(code) << 48) | (static_cast<unsigned long long>(blockIdx.x) << 32) | (static_cast<unsigned>(a) & 0xffffu) << 16 | (static_cast<unsigned>(b) & 0xffffu); __threadfence_system(); }
+    if (gtime() - t0 > (code == 7 || code == 8 ? 1000000000ull : 2000000000ull)) {
+      if (dbg && atomicCAS(dbg + 2, 0ull, 1ull) == 0ull) { dbg[1] = (static_cast<unsigned long long>(static_cast<unsigned>(a)) << 32) | static_cast<unsigned>(b); dbg[0] = (static_cast<unsigned long long>(code) << 48) | (static_cast<unsigned long long>(blockIdx.x) << 32) | (static_cast<unsigned>(a) & 0xffffu) << 16 | (static_cast<unsigned>(b) & 0xffffu); __threadfence_system(); }
       __trap();
     }
   }
@@ -166,6 +175,16 @@ struct Watch {
 #else
 #define ART_WATCH(name, code)
 #define ART_WATCH_POLL(name, ...)
+#endif
+
+#ifdef ART_PC_STATS
+#define ART_STAT_ADD(i, v) do { if (pp.stats && lane == 0) atomicAdd(pp.stats + (i), static_cast<unsigned long long>(v)); } while (0)
+#define ART_STAT_T(name) const long long name = clock64()
+#define ART_STAT_SET(name) name = clock64()
+#else
+#define ART_STAT_SET(name)
+#define ART_STAT_ADD(i, v)
+#define ART_STAT_T(name)
 #endif
 
 // self-validating words: the lowest mantissa bit carries the generation parity of the slot; -inf travels as -1e30
@@ -184,7 +203,8 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
   constexpr bool kTwoPBufs = (G == 8 && MODE == 1);
   constexpr uint32_t SUMB = sum_bytes(G, PW);
   constexpr int PF = G * (kD + 2);                       // floats of one partial state
-  using Scan = ChunkScan<G, PW>;
+  constexpr int GW = G >= 8 ? 2 : 1;                     // heads per scanning warp (the fold warps of the home CTA scan)
+  using Scan = ChunkScan<GW, PW>;
   const Params& p = pp.b;
 
   extern __shared__ __align__(1024) uint8_t smem[];
@@ -194,7 +214,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
   if ((sbase & 1023u) != 0u) __trap();
   const uint32_t bars = sbase + sm.bars;
   auto bar = [&](uint32_t idx) { return bars + idx * 8u; };
-  IterSlot* slots = reinterpret_cast<IterSlot*>(smem + sm.slots);
+  float* slots = reinterpret_cast<float*>(smem + sm.slots);   // [item & 15][2 G]: block maximum (log2 domain), block sum
   volatile Item* items = reinterpret_cast<volatile Item*>(smem + sm.items);
   const uint32_t a_misc = sbase + sm.misc;
 
@@ -291,7 +311,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     v_tr = make_trav(p, v_b, v_g, v_L); v_T = v_tr.T;
   };
   // become the home of local group i (lane-uniform); false if the group is empty (handled here)
-  auto open_group = [&](int i) -> bool {
+  auto open_group = [&](int i, bool before_start) -> bool {
     set_group(cidx + i * pp.NC);
     if (v_T == 0) {                                        // no eligible block: out = 0, t* = 0
       for (int o = lane; o < p.Gr * kD; o += 32) {
@@ -305,12 +325,14 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     v_hs = rank * 2 + hsl; v_gen = my_gen & 127;
     if (lane == 0) {
       ART_WATCH(wd, 1);
-      while (atom_cas_cluster_acqrel(board_at(v_hs, B_NACT), 0, kLock) != 0) { nsleep(64); ART_WATCH_POLL(wd, v_hs, my_gen); }
+      while (atom_cas_cluster_acquire(board_at(v_hs, B_NACT), 0, kLock) != 0) { nsleep(64); ART_WATCH_POLL(wd, v_hs, my_gen); }
     }
     __syncwarp();
     if constexpr (ART) {                                   // nobody is left who could still write a notice of the slot's last group
       uint32_t* tg = reinterpret_cast<uint32_t*>(smem + sm.tags) + hsl * kNR;
       for (int i2 = lane; i2 < kNR; i2 += 32) tg[i2] = 0u;
+      uint32_t* sb = reinterpret_cast<uint32_t*>(smem + sm.stab) + hsl * kNR;      // four scanning warps x kNR bytes
+      for (int i2 = lane; i2 < kNR; i2 += 32) sb[i2] = 0u;
     }
     if (lane == 0) {
       HomeInfo* hi = reinterpret_cast<HomeInfo*>(smem + sm.hinfo) + hsl;
@@ -323,7 +345,9 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     }
     __syncwarp();
     if (lane == 0) {
-      atom_add_cluster_acqrel(board_at(v_hs, B_NACT), 1 - kLock);     // open, one worker (this CTA); releases all of the above
+      // open, one worker (this CTA); releases all of the above (before the start the cluster barrier does that)
+      if (before_start) atom_add_cluster(board_at(v_hs, B_NACT), 1 - kLock);
+      else atom_add_cluster_release(board_at(v_hs, B_NACT), 1 - kLock);
       if constexpr (ART) asm volatile("st.release.cta.shared::cta.s32 [%0], %1;" :: "r"(a_misc + kMOpen), "r"(my_gen + 1) : "memory");
     }
     __syncwarp();
@@ -358,12 +382,12 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     if (best == 0) return false;
     int ok = 0, T2 = 0, grp = 0, gen2 = 0;
     if (lane == 0) {
-      const int old = atom_add_cluster_acqrel(board_at(who, B_NACT), 1);        // pin: the slot cannot be reopened under us
+      const int old = atom_add_cluster_acquire(board_at(who, B_NACT), 1);       // pin: the slot cannot be reopened under us
       T2 = ld_cluster_relaxed_s32(board_at(who, B_T)); grp = ld_cluster_relaxed_s32(board_at(who, B_GROUP));
       gen2 = ld_cluster_relaxed_s32(board_at(who, B_GEN));
       const int nx = ld_cluster_relaxed_s32(board_at(who, B_NEXT));
       ok = (old > 0 && grp >= 0 && nx < T2) ? 1 : 0;
-      if (!ok) atom_add_cluster_acqrel(board_at(who, B_NACT), -1);
+      if (!ok) atom_add_cluster(board_at(who, B_NACT), -1);
     }
     ok = __shfl_sync(0xffffffffu, ok, 0);
     if (!ok) return true;                                  // lost a race: look again
@@ -373,11 +397,22 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     return true;
   };
   // leave the current group without having issued an item for it
-  auto leave_quietly = [&]() { if (lane == 0) atom_add_cluster_acqrel(board_at(v_hs, B_NACT), -1); __syncwarp(); };
+  auto leave_quietly = [&]() { if (lane == 0) atom_add_cluster(board_at(v_hs, B_NACT), -1); __syncwarp(); };
 
-  if (warp == kWarpProducer && rank < n_init) have = open_group(rank);
+  if (warp == kWarpProducer && rank < n_init) have = open_group(rank, true);
   // every CTA's first group is on the board before anybody looks for a group to join
   cluster_sync_all();
+  if (warp == kWarpProducer && rank >= n_init && n_init > 0) {
+    // the CTAs that opened nothing start as workers of the cluster's first groups, dealt round-robin: no search
+    const int home = rank % n_init;
+    set_group(cidx + home * pp.NC);
+    if (v_T >= kMinJoin) {                                  // (an empty or tiny first group: look for work the usual way)
+      v_hs = home * 2; v_gen = 0;
+      if (lane == 0) atom_add_cluster(board_at(v_hs, B_NACT), 1);
+      __syncwarp();
+      have = true;
+    }
+  }
 
   if (warp == kWarpProducer) {
     // ===================================================== A1 + A2: claim steps, resolve blocks, issue TMA loads
@@ -387,7 +422,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
           int i = 0;
           if (lane == 0) i = atom_add_cluster(a_next_local, 1);
           i = __shfl_sync(0xffffffffu, i, 0);
-          if (i < n_local) { have = open_group(i); if (!have) continue; }
+          if (i < n_local) { have = open_group(i, false); if (!have) continue; }
           else more_local = false;
         }
         if (!have) {
@@ -402,7 +437,18 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
       }
       // ---- the visit: claim steps until the group has none left (or Algorithm 1 has fired)
       const uint32_t a_next = board_at(v_hs, B_NEXT), a_nact = board_at(v_hs, B_NACT);
-      auto claim = [&]() -> int { return atom_add_cluster(a_next, 1) + 1; };
+      // steps are claimed a chunk of `claim` consecutive steps at a time, one chunk ahead of the one being issued,
+      // so the round trip to the board is never waited for
+      const int K = pp.claim;
+      int ch_t = 0, ch_left = 0, nx = 0, nactB = 1;
+      auto claim_chunk = [&]() {
+        if (lane == 0) { nx = atom_add_cluster(a_next, K) + 1; if constexpr (ART) nactB = ld_cluster_relaxed_s32(a_nact); }
+      };
+      auto next_step = [&]() -> int {
+        if (ch_left == 0) { ch_t = __shfl_sync(0xffffffffu, nx, 0); ch_left = K; if (ch_t <= v_T) claim_chunk(); }
+        --ch_left;
+        return ch_t++;
+      };
       auto resolve = [&](int t, bool& valid, unsigned long long& mask, int& page, int& ec) {
         bool fired = false;
         if constexpr (ART) read_ctrl(v_hs, v_gen, fired);
@@ -415,24 +461,24 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
           if (mask) page = p.block_table[static_cast<int64_t>(v_b) * p.max_blocks + blk];
         }
       };
-      int tB = 0, nactB = 1;
-      if (lane == 0) tB = claim();
-      int tA = __shfl_sync(0xffffffffu, tB, 0);
+      claim_chunk();
+      int tA = next_step();
       bool validA; unsigned long long maskA; int pageA, ecA;
       resolve(tA, validA, maskA, pageA, ecA);
-      if (lane == 0 && validA) { tB = claim(); if constexpr (ART) nactB = ld_cluster_relaxed_s32(a_nact); }
       while (validA) {
-        const int tN = __shfl_sync(0xffffffffu, tB, 0);
+        const int tN = next_step();
         bool validB; unsigned long long maskB; int pageB, ecB;
         resolve(tN, validB, maskB, pageB, ecB);
-        if (validB && lane == 0) { tB = claim(); if constexpr (ART) nactB = ld_cluster_relaxed_s32(a_nact); }
         if constexpr (ART) {
           // A7 / run-ahead: the loads of step t go out once step t - R is decided (R grows with the workers of the group)
           int R = pp.rw * max(__shfl_sync(0xffffffffu, nactB, 0), 1);
           R = R > kNR ? kNR : R;
           bool fired = false;
           ART_WATCH(wd, 2);
-          while (read_ctrl(v_hs, v_gen, fired) < tA - R && !fired) { ART_WATCH_POLL(wd, v_hs, tA); }
+          ART_STAT_T(tg0);
+          while (read_ctrl(v_hs, v_gen, fired) < tA - R && !fired) { nsleep(pp.nap); ART_WATCH_POLL(wd, v_hs, tA); }
+          ART_STAT_T(tg1);
+          ART_STAT_ADD(8, tg1 - tg0); ART_STAT_ADD(10, 1);
           if (fired) break;                                  // t > t*: nothing of this group is loaded any more
         }
         if (v_items == 0) {
@@ -449,7 +495,10 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
           __syncwarp();
           ++nvisit;
         }
+        ART_STAT_T(te0);
         wait_empty();
+        ART_STAT_T(te1);
+        ART_STAT_ADD(9, te1 - te0);
         if (lane == 0) {
           const uint32_t fb = bar(sm.full0 + stage);
           const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
@@ -557,12 +606,183 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     const int q = warp - kWarpSoftmax0;
     const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
     int st = q % S;
+    // ---- home duty (ART on).  The softmax warps are idle most of the time and carry no state from item to item, so
+    //      they replay Algorithm 1 for the group this CTA opened: warp w scans heads w GW .. w GW + GW - 1
+    //      (art_scan_chunk.cuh) and leaves one byte per step in `stab`; warp 0 also walks the patience counter over
+    //      those bytes and broadcasts the progress word.  One call does at most one chunk; true if it did something.
+      constexpr int LPH = Scan::LPH, CPL = Scan::CPL, NBK = Scan::NBK, STRIDE = Scan::STRIDE;
+      constexpr int NSW = G / GW;                             // warps that have heads to scan
+      const int fw = warp - kWarpSoftmax0;                    // softmax warp w scans heads w GW .. w GW + GW - 1
+      const int sub = lane % LPH, h_scan = fw * GW + lane / LPH;   // the head this lane scans
+      const bool owner = (sub % STRIDE) == 0;
+      const int own_k = sub / STRIDE;
+      const bool i_scan = fw < NSW && fw * GW < p.Gr;         // this warp has at least one real head
+      const int nsw_real = (p.Gr + GW - 1) / GW;              // warps whose bytes the decider waits for
+      int sg = 0;                                             // groups of this home CTA already scanned
+      bool scanning = false;
+      int s_t = 1, s_T = 0, s_gen = 0, s_group = 0, s_hs = 0; // the group being scanned: next step, ...
+      int d_t = 0, d_cnt = 0;                                 // warp 0: last decided step, c^(t)
+      Scan sc; sc.init(true);
+      // a chunk whose summaries are on their way over distributed shared memory (issued at the top of an iteration,
+      // looked at after the item work of the same iteration: the round trip hides behind it)
+      int pend_n = 0;
+      long long pend_t0 = 0; (void)pend_t0;
+      uint32_t pend_word = 0u, pend_ml[2] = {0u, 0u}, pend_raw[NBK][CPL];
+      auto issue_pull = [&]() {
+        const uint32_t wk_own = __shfl_sync(0xffffffffu, pend_word, own_k);
+        if (owner && own_k < pend_n)
+          ld_cluster_vec<2>(mapa(sbase + sm.sums + (wk_own & 7u) * SUMB, (wk_own >> 4) & 15u) + static_cast<uint32_t>(G * PW + 2 * h_scan) * 4u, pend_ml);
+#pragma unroll
+        for (int k = 0; k < NBK; ++k) {
+          const uint32_t wk = __shfl_sync(0xffffffffu, pend_word, k);
+          if (k < pend_n) ld_cluster_vec<CPL>(mapa(sbase + sm.sums + (wk & 7u) * SUMB, (wk >> 4) & 15u) + static_cast<uint32_t>(h_scan * PW + sub * CPL) * 4u, pend_raw[k]);
+        }
+      };
+      // which of the next NBK steps have arrived (lane k looks at step first + k)?  Issue the loads of their summaries.
+      auto poll_and_pull = [&](int first) {
+        const uint32_t tg = sbase + sm.tags + static_cast<uint32_t>(s_hs & 1) * kNR * 4u;
+        bool ok = false;
+        pend_word = 0u;
+        if (lane < NBK && first + lane <= s_T) {
+          pend_word = static_cast<uint32_t>(ld_volatile_s32(tg + static_cast<uint32_t>((first + lane - 1) % kNR) * 4u));
+          ok = (pend_word >> 8) == static_cast<uint32_t>(first + lane);
+        }
+        pend_n = __ffs(~__ballot_sync(0xffffffffu, ok)) - 1;
+        if (pend_n > 0) { issue_pull(); ART_STAT_SET(pend_t0); }
+      };
+      auto scan_duty = [&]() -> bool {
+        bool progress = false;
+        // ---- (3) home duty
+        if (!scanning) {
+          int oc;
+          asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(oc) : "r"(a_misc + kMOpen) : "memory");
+          if (oc > sg) {
+            const HomeInfo* hi = reinterpret_cast<const HomeInfo*>(smem + sm.hinfo) + (sg & 1);
+            s_group = *reinterpret_cast<const volatile int*>(&hi->group); s_T = *reinterpret_cast<const volatile int*>(&hi->T);
+            s_gen = *reinterpret_cast<const volatile int*>(&hi->gen);
+            s_hs = rank * 2 + (sg & 1); s_t = 1; d_t = 0; d_cnt = 0;
+            sc.init(h_scan < p.Gr);
+            scanning = true;
+          }
+        }
+        if (scanning) {
+          const int hsl = s_hs & 1;
+          bool fin_seen;
+          const int g_dec = read_ctrl(s_hs, s_gen, fin_seen);
+          fin_seen = fin_seen || g_dec >= s_T;
+          if (fin_seen) { scanning = false; pend_n = 0; ++sg; progress = true; }
+          else if (i_scan && pend_n == 0 && s_t <= s_T) { poll_and_pull(s_t); progress = pend_n > 0; }
+          else if (pend_n > 0) {
+            // ---- (3b) the chunk's summaries are here.  A word whose parity bit is the slot's previous generation's
+            //      (written by another warp of the producing CTA a moment later): pull again.
+            int n = pend_n;
+            const uint32_t wk_own = __shfl_sync(0xffffffffu, pend_word, own_k);
+            const bool has_own = owner && own_k < n;
+            uint32_t bad = has_own ? ((pend_ml[0] ^ (wk_own >> 3)) | (pend_ml[1] ^ (wk_own >> 3))) : 0u;
+            float pv[NBK][CPL];
+#pragma unroll
+            for (int k = 0; k < NBK; ++k) {
+              const uint32_t pk = __shfl_sync(0xffffffffu, pend_word, k) >> 3;
+#pragma unroll
+              for (int j = 0; j < CPL; ++j) {
+                if (k < n) { bad |= pend_raw[k][j] ^ pk; pv[k][j] = __uint_as_float(pend_raw[k][j]); }
+                else pv[k][j] = 0.f;
+              }
+            }
+            if (__any_sync(0xffffffffu, (bad & 1u) != 0u)) {
+              if (fw == 0) ART_STAT_ADD(4, 1);
+              issue_pull();                                   // (if Algorithm 1 has fired meanwhile, fin_seen ends this next time round)
+            } else {
+              float m_own = kNegInf, l_own = 0.f;
+              if (has_own) { m_own = __uint_as_float(pend_ml[0]); l_own = __uint_as_float(pend_ml[1]); if (m_own <= -1e29f) m_own = kNegInf; }
+              if (n > 1 && !sc.spread_ok(m_own, owner)) {     // exponents too far apart for one reference: one step at a time
+                n = 1;
+                if (own_k >= 1) { m_own = kNegInf; l_own = 0.f; }
+#pragma unroll
+                for (int k = 1; k < NBK; ++k)
+#pragma unroll
+                  for (int j = 0; j < CPL; ++j) pv[k][j] = 0.f;
+              }
+              // the next chunk's summaries travel while this one is scanned
+              const int first = s_t;
+              s_t += n;
+              pend_n = 0;
+              if (s_t <= s_T) poll_and_pull(s_t);
+              ART_STAT_T(tc0);
+              const uint32_t bits = sc.chunk(n, lane, p.tau, p.phi, m_own, l_own, pv);
+              ART_STAT_T(tc1);
+              if (fw == 0) { ART_STAT_ADD(0, 1); ART_STAT_ADD(1, n); ART_STAT_ADD(2, tc0 - pend_t0); ART_STAT_ADD(3, tc1 - tc0); }
+              // one byte per step: [lap tag : 7][stable : 1]
+              if (lane < n) {
+                const int s = first + lane;
+                const uint32_t byte = (static_cast<uint32_t>(((s - 1) / kNR) % 127 + 1) << 1) | ((bits >> lane) & 1u);
+                *reinterpret_cast<volatile uint8_t*>(smem + sm.stab + (hsl * 4 + fw) * kNR + (s - 1) % kNR) = static_cast<uint8_t>(byte);
+              }
+            }
+            progress = true;
+          }
+          if (fw == 0 && !fin_seen) {
+            // ---- the patience counter (Eq. 3) over the steps every scanning warp has finished
+            bool valid = false, stable = true;
+            const int s = d_t + 1 + lane;
+            if (lane < 16 && s <= s_T) {
+              const uint32_t want = static_cast<uint32_t>(((s - 1) / kNR) % 127 + 1);
+              valid = true;
+              for (int w = 0; w < nsw_real; ++w) {
+                const uint32_t b8 = *reinterpret_cast<volatile uint8_t*>(smem + sm.stab + (hsl * 4 + w) * kNR + (s - 1) % kNR);
+                valid = valid && (b8 >> 1) == want;
+                stable = stable && (b8 & 1u);
+              }
+            }
+            const int nv = __ffs(~__ballot_sync(0xffffffffu, valid)) - 1;
+            if (nv > 0) {
+              const uint32_t sb = __ballot_sync(0xffffffffu, stable);
+              int fired_at = 0;
+              for (int k = 0; k < nv && !fired_at; ++k) {
+                d_cnt = ((sb >> k) & 1u) ? d_cnt + 1 : 0;     // Eq. 3
+                if (d_cnt >= p.patience) fired_at = d_t + 1 + k;
+              }
+              d_t = fired_at ? fired_at : d_t + nv;
+              const uint32_t a_c = sbase + sm.ctrl + static_cast<uint32_t>(s_hs) * 4u;
+              if (fired_at || d_t >= s_T) {
+                // t* is known: record it, let the last flusher recognise itself, THEN release the final progress word
+                if (lane == 0) {
+                  p.stop_block[s_group] = d_t;               // t* (R9)
+                  asm volatile("red.relaxed.cluster.shared::cluster.add.u64 [%0], %1;" :: "r"(hinfo_at(s_hs, H_DONE)), "l"(static_cast<unsigned long long>(d_t + 1) << 32) : "memory");
+                }
+                __syncwarp();
+                if (lane < CL) st_cluster_release_s32(mapa(a_c, lane), ctrl_word(s_gen, fired_at != 0, d_t));
+              } else if (lane < CL) {
+                st_cluster_relaxed_s32(mapa(a_c, lane), ctrl_word(s_gen, false, d_t));
+              }
+              progress = true;
+            }
+          }
+        }
+        return progress;
+      };
+      // true once no group is left for this CTA to scan
+      auto scan_all_done = [&]() -> bool {
+        if (scanning || !ld_volatile_s32(a_misc + kMScanExit)) return false;
+        int oc;
+        asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(oc) : "r"(a_misc + kMOpen) : "memory");
+        return oc <= sg;
+      };
     for (int i = q;; i += NS) {
-      mbar_wait(bar(sm.sfull0 + q), (i / NS) & 1);
+      if constexpr (ART) {
+        ART_WATCH(wds, 7);
+        while (!mbar_test_wait(bar(sm.sfull0 + q), (i / NS) & 1)) { if (!scan_duty()) nsleep(pp.nap); if (scanning) ART_WATCH_POLL(wds, s_t, (d_t << 8) | (pend_n << 4) | (scanning ? 1 : 0) | (q << 1)); }
+      } else {
+        mbar_wait(bar(sm.sfull0 + q), (i / NS) & 1);
+      }
       const int kind = item_kind(items[i % kItemsRing].meta);
       if (kind == ITEM_END) {
         // the END item that owns a stage is the first of the four; only its warp hands it on to the P.V issuer
         if (item_kind(items[(i + kItemsRing - 1) % kItemsRing].meta) != ITEM_END || i == 0) mbar_arrive(bar(sm.pfull0 + st));
+        if constexpr (ART) {                                  // no item left; the group(s) this CTA opened may still run
+          ART_WATCH(wde, 8);
+          while (!scan_all_done()) { if (!scan_duty()) nsleep(pp.nap); ART_WATCH_POLL(wde, s_t, (d_t << 8) | (pend_n << 4) | (scanning ? 1 : 0) | (q << 1)); }
+        }
         break;
       }
       if (kind != ITEM_DATA) {                               // a marker: nothing to compute
@@ -633,8 +853,8 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
         float mine = mb[0];
 #pragma unroll
         for (int h = 1; h < G; ++h) mine = (hh == h) ? mb[h] : mine;
-        IterSlot& slot = slots[i & (kIterSlots - 1)];
-        if ((lane & (32 / G - 1)) == 0) { slot.mref[hh] = mine; slot.lsum[hh] = ls[0]; }
+        float* slot = slots + (i & (kIterSlots - 1)) * 2 * G;
+        if ((lane & (32 / G - 1)) == 0) { slot[hh] = mine; slot[G + hh] = ls[0]; }
       }
       fence_proxy_async();
       mbar_arrive(bar(sm.pfull0 + st));
@@ -661,85 +881,113 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
       float pv[G];
       tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN, pv);
       tmem_ld_wait();
-      const IterSlot& sl = slots[i & (kIterSlots - 1)];
+      const float* sl = slots + (i & (kIterSlots - 1)) * 2 * G;
 #pragma unroll
       for (int h = 0; h < G; ++h) {
-        const float mr = sl.mref[h];
+        const float mr = sl[h];
         if (mr != kNegInf) {                                  // a block with no valid token changes nothing
           const float mn = fmaxf(m_tot[h], mr);
           const float a = fast_exp2(m_tot[h] - mn), bb = fast_exp2(mr - mn);
           acc[h] = fmaf(a, acc[h], bb * pv[h]);
-          l_tot[h] = fmaf(a, l_tot[h], bb * sl.lsum[h]);
+          l_tot[h] = fmaf(a, l_tot[h], bb * sl[G + h]);
           m_tot[h] = mn;
         }
       }
       ++nfold;
       release_pv(i);
     };
-    // out[row h] = combination of the partial states of the CTAs in `joined` (flash-decoding merge)
-    auto combine = [&](int group, unsigned joined, int T) {
+    // out[row h] = our own partial state (registers) merged with the flushed partial states of the CTAs in `others`
+    // (flash-decoding merge).  The partial states are read a few at a time with every load of a
+    // batch in flight at once: the combine sits on the tail of the call.
+    auto combine = [&](int group, unsigned others, int T) {
       const int b = group / p.Hkv, g = group % p.Hkv;
-      const bool alone = joined == (1u << rank);
+      constexpr int CH = G <= 2 ? 4 : (G <= 4 ? 3 : 2);
+      float mx[G], a[G], l[G];
 #pragma unroll
-      for (int h = 0; h < G; ++h) {
-        float a = acc[h], l = l_tot[h];
-        if (!alone) {
-          float mx = kNegInf;
-          for (unsigned js = joined; js; js &= js - 1) {
-            const int c = __ffs(js) - 1;
-            mx = fmaxf(mx, __ldcg(pp.part + (static_cast<size_t>(group) * CL + c) * PF + G * kD + h));
-          }
-          a = 0.f; l = 0.f;
-          for (unsigned js = joined; js; js &= js - 1) {
-            const int c = __ffs(js) - 1;
-            const float* pc = pp.part + (static_cast<size_t>(group) * CL + c) * PF;
-            const float mc = __ldcg(pc + G * kD + h);
-            const float f = (mc == kNegInf) ? 0.f : fast_exp2(mc - mx);
-            a = fmaf(f, __ldcg(pc + h * kD + d), a);
-            l = fmaf(f, __ldcg(pc + G * kD + G + h), l);
-          }
+      for (int h = 0; h < G; ++h) { mx[h] = m_tot[h]; a[h] = acc[h]; l[h] = l_tot[h]; }
+      unsigned js = others;
+      while (js) {
+        const float* pc[CH];
+#pragma unroll
+        for (int k = 0; k < CH; ++k) {
+          pc[k] = nullptr;
+          if (js) { pc[k] = pp.part + (static_cast<size_t>(group) * CL + (__ffs(js) - 1)) * PF; js &= js - 1; }
         }
-        if (h < p.Gr)                                         // Alg. 1 l.18; row h = query token h / Gh, head h % Gh
-          p.out[((static_cast<int64_t>(b) * p.qlen + h / p.Gh) * p.Hq + g * p.Gh + h % p.Gh) * kD + d] = (l > 0.f) ? a / l : 0.f;
+        float mc[CH][G], lc[CH][G], ac[CH][G];
+#pragma unroll
+        for (int k = 0; k < CH; ++k)
+#pragma unroll
+          for (int h = 0; h < G; ++h) {
+            mc[k][h] = pc[k] ? __ldcg(pc[k] + G * kD + h) : kNegInf;
+            lc[k][h] = pc[k] ? __ldcg(pc[k] + G * kD + G + h) : 0.f;
+            ac[k][h] = pc[k] ? __ldcg(pc[k] + h * kD + d) : 0.f;
+          }
+#pragma unroll
+        for (int k = 0; k < CH; ++k)
+#pragma unroll
+          for (int h = 0; h < G; ++h) {
+            if (mc[k][h] != kNegInf) {
+              const float mn = fmaxf(mx[h], mc[k][h]);
+              const float f0 = fast_exp2(mx[h] - mn), f1 = fast_exp2(mc[k][h] - mn);
+              a[h] = fmaf(f0, a[h], f1 * ac[k][h]);
+              l[h] = fmaf(f0, l[h], f1 * lc[k][h]);
+              mx[h] = mn;
+            }
+          }
       }
+#pragma unroll
+      for (int h = 0; h < G; ++h)
+        if (h < p.Gr)                                         // Alg. 1 l.18; row h = query token h / Gh, head h % Gh
+          p.out[((static_cast<int64_t>(b) * p.qlen + h / p.Gh) * p.Hq + g * p.Gh + h % p.Gh) * kD + d] = (l[h] > 0.f) ? a[h] / l[h] : 0.f;
       if (!ART && d == 0) p.stop_block[group] = T;
     };
-    // end of a visit: hand the partial state over, combine if we are the last, leave the group
+    // End of a visit: hand the partial state over, combine if we are the last, leave the group.
+    //   done word of the group (home CTA): low half = steps folded AND flushed so far, high half = t* + 1 once known.
+    //   Whoever brings the low half to t* combines.  A CTA that finds itself the group's only worker ever (nobody
+    //   else is working on it, nobody has flushed, all t* steps are in its registers) skips the round trip.
     auto flush = [&](int tcode, int meta, unsigned long long payload) {
       const int hs = item_hs(meta), group = static_cast<int>(payload);
-      if (nfold > 0) {
+      if (warp == kWarpFold0 && lane == 0) {
+        int flag = 0;                                         // 0: not ours to combine; 1: alone; >= 2: last of several, t* + 1
+        if (p.blocks_loaded && tcode > 0) atomicAdd(p.blocks_loaded + group, tcode);
+        if (nfold > 0) {
+          const int nact = ld_cluster_relaxed_s32(board_at(hs, B_NACT));
+          const unsigned jn = ld_cluster_u32(hinfo_at(hs, H_JOINED));
+          unsigned long long dn;
+          asm volatile("ld.relaxed.cluster.shared::cluster.u64 %0, [%1];" : "=l"(dn) : "r"(hinfo_at(hs, H_DONE)) : "memory");
+          if (nact == 1 && jn == 0u && static_cast<unsigned>(dn) == 0u && static_cast<unsigned>(dn >> 32) == static_cast<unsigned>(nfold) + 1u) flag = 1;
+        }
+        st_volatile_s32(a_misc + kMFlag, flag);
+        st_volatile_s32(a_misc + kMJoined, 0);
+      }
+      named_bar_sync(1, 128);
+      int flag = ld_volatile_s32(a_misc + kMFlag);
+      if (flag == 0 && nfold > 0) {
         float* part = pp.part + (static_cast<size_t>(group) * CL + rank) * PF;
 #pragma unroll
         for (int h = 0; h < G; ++h) {
           part[h * kD + d] = acc[h];
           if (d == 0) { part[G * kD + h] = m_tot[h]; part[G * kD + G + h] = l_tot[h]; }
         }
-        __threadfence();
-      }
-      named_bar_sync(1, 128);
-      if (warp == kWarpFold0 && lane == 0) {
-        int flag = 0;
-        if (p.blocks_loaded && tcode > 0) atomicAdd(p.blocks_loaded + group, tcode);
-        if (nfold > 0) {
-          atom_or_cluster(hinfo_at(hs, H_JOINED), 1u << rank);
+        named_bar_sync(1, 128);                               // every thread's part is written ...
+        if (warp == kWarpFold0 && lane == 0) {
+          const unsigned before = atom_or_cluster(hinfo_at(hs, H_JOINED), 1u << rank);
+          // ... and released by this one atomic (cumulative over the barrier); acquire: the partial states of the others
           const unsigned long long old = atom_add64_cluster_acqrel(hinfo_at(hs, H_DONE), static_cast<unsigned long long>(nfold));
           const unsigned long long tot = old + static_cast<unsigned long long>(nfold);
           const unsigned hi = static_cast<unsigned>(tot >> 32), lo = static_cast<unsigned>(tot);
           if (hi != 0u && lo == hi - 1u) {                    // every step <= t* is folded and flushed: we combine
-            flag = static_cast<int>(hi);
-            st_volatile_s32(a_misc + kMJoined, static_cast<int>(ld_cluster_u32(hinfo_at(hs, H_JOINED))));
+            st_volatile_s32(a_misc + kMJoined, static_cast<int>((before | ld_cluster_u32(hinfo_at(hs, H_JOINED))) & ~(1u << rank)));
+            st_volatile_s32(a_misc + kMFlag, static_cast<int>(hi));      // >= 2: t* + 1
           }
         }
-        st_volatile_s32(a_misc + kMFlag, flag);
+        named_bar_sync(1, 128);
+        flag = ld_volatile_s32(a_misc + kMFlag);
       }
-      named_bar_sync(1, 128);
-      const int flag = ld_volatile_s32(a_misc + kMFlag);
-      if (flag) {
-        __threadfence();
-        combine(group, static_cast<unsigned>(ld_volatile_s32(a_misc + kMJoined)), flag - 1);
-      }
-      named_bar_sync(1, 128);                                 // the flag is read by all before the next flush rewrites it
-      if (warp == kWarpFold0 && lane == 0) atom_add_cluster_acqrel(board_at(hs, B_NACT), -1);   // leave (after everything above)
+      if (flag) combine(group, static_cast<unsigned>(ld_volatile_s32(a_misc + kMJoined)), flag == 1 ? nfold : flag - 1);
+      named_bar_sync(1, 128);                                 // flag and mask are read by all before the next flush rewrites them
+      // leave; the release orders our notices before a re-opening of the slot can clear its notice ring
+      if (warp == kWarpFold0 && lane == 0) { if constexpr (ART) atom_add_cluster_release(board_at(hs, B_NACT), -1); else atom_add_cluster(board_at(hs, B_NACT), -1); }
       reset_state();
     };
 
@@ -754,29 +1002,33 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
         release_pv(i);
       }
     } else {
+      // ---- ART on: (1) merge or drop the oldest finished item once its step is decided, (2) write the summary of the
+      //      next finished item and tell its group's home.  Neither waits for the other.
+      constexpr int LPH = Scan::LPH, CPL = Scan::CPL;
       int pub = 0, fld = 0;
-      bool pub_ready = false;
+      bool pub_ready = false, items_done = false;
       ART_WATCH(wd, 3);
-      for (;;) {
-        // ---- the oldest unfolded item: merge it once its step is decided, drop it if it lies beyond t*
-        if (fld < pub) {
+      while (!items_done) {
+        bool progress = false;
+        // ---- (1) the oldest unfolded item
+        if (!items_done && fld < pub) {
           const int meta = items[fld % kItemsRing].meta;
           const int kind = item_kind(meta);
           if (kind == ITEM_DATA) {
             bool fired;
             const int tdec = read_ctrl(item_hs(meta), item_gen(meta), fired);
             const int tf = items[fld % kItemsRing].tcode & kItemStep;
-            if (fired && tf > tdec) { release_pv(fld); ++fld; continue; }
-            if (tdec >= tf) { fold(fld); ++fld; continue; }   // decided: the scan has read this step's summary
+            if (fired && tf > tdec) { release_pv(fld); ++fld; progress = true; }
+            else if (tdec >= tf) { fold(fld); ++fld; progress = true; }   // decided: the scan has read this step's summary
           } else if (kind == ITEM_FLUSH) {
             flush(items[fld % kItemsRing].tcode, meta, items[fld % kItemsRing].mask);
-            release_pv(fld); ++fld; continue;
+            release_pv(fld); ++fld; progress = true;
           } else {
-            break;                                            // END
+            items_done = true;                                // END: only the home duty may be left
           }
         }
-        // ---- the next finished item: write its summary, tell the group's home where it is
-        if (pub - fld < NSUM) {
+        // ---- (2) the next finished item: write its summary, tell the group's home where it is
+        if (!items_done && pub - fld < NSUM) {
           const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
           const uint32_t par = (pub / NP) & 1;
           if (!pub_ready) pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
@@ -793,16 +1045,15 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
               uint32_t* sw = reinterpret_cast<uint32_t*>(smem + sm.sums + sslot * SUMB);
               if (MODE == 2 || (d & 3) == 0) {
                 const int pi = (MODE == 2) ? d : (d >> 2);    // probe coordinate k * (d / 32)  (R1)
-                const int sub = pi % Scan::LPH, j = pi / Scan::LPH;
 #pragma unroll
-                for (int h = 0; h < G; ++h) sw[(h * Scan::LPH + sub) * Scan::CPL + j] = tag_word(pv[h], gpar);
+                for (int h = 0; h < G; ++h) sw[h * PW + (pi % LPH) * CPL + pi / LPH] = tag_word(pv[h], gpar);
               }
               if (d == 1) {
-                const IterSlot& sl = slots[pub & (kIterSlots - 1)];
+                const float* sl = slots + (pub & (kIterSlots - 1)) * 2 * G;
 #pragma unroll
                 for (int h = 0; h < G; ++h) {
-                  sw[G * PW + 2 * h] = tag_word(fmaxf(sl.mref[h], kNegBig), gpar);
-                  sw[G * PW + 2 * h + 1] = tag_word(sl.lsum[h], gpar);
+                  sw[G * PW + 2 * h] = tag_word(fmaxf(sl[h], kNegBig), gpar);
+                  sw[G * PW + 2 * h + 1] = tag_word(sl[G + h], gpar);
                 }
               }
               __syncwarp();
@@ -816,120 +1067,11 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
                 }
               }
             }
-            ++pub; pub_ready = false;
-            continue;
+            ++pub; pub_ready = false; progress = true;
           }
         }
-        ART_WATCH_POLL(wd, fld, pub);
+        if (!progress && fld < pub) { nsleep(pp.nap); ART_WATCH_POLL(wd, items[fld % kItemsRing].tcode, ld_ctrl_relaxed(sbase + sm.ctrl + static_cast<uint32_t>(item_hs(items[fld % kItemsRing].meta)) * 4u)); }
       }
-    }
-  } else if (ART && warp == kWarpScan) {
-    // ===================================================== A6 + A7 + A9: Algorithm 1 over step summaries (home of a group)
-    constexpr int LPH = Scan::LPH, CPL = Scan::CPL, NBK = Scan::NBK, STRIDE = Scan::STRIDE;
-    const int sub = lane % LPH;
-    const bool owner = (sub % STRIDE) == 0;
-    const int own_k = sub / STRIDE;                          // the step of a chunk this lane owns for its head
-    const int h_lane = lane / LPH;
-    int sg = 0;
-    for (;;) {
-      {
-        ART_WATCH(wd, 4);
-        bool stop = false;
-        for (;;) {
-          int oc;
-          asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(oc) : "r"(a_misc + kMOpen) : "memory");
-          if (oc > sg) break;
-          if (ld_volatile_s32(a_misc + kMScanExit)) {
-            asm volatile("ld.acquire.cta.shared::cta.s32 %0, [%1];" : "=r"(oc) : "r"(a_misc + kMOpen) : "memory");
-            if (oc > sg) break;
-            stop = true; break;
-          }
-          nsleep(100);
-          ART_WATCH_POLL(wd, sg, 0);
-        }
-        if (stop) break;
-      }
-      const int hsl = sg & 1, hs = rank * 2 + hsl;
-      const HomeInfo* hi = reinterpret_cast<const HomeInfo*>(smem + sm.hinfo) + hsl;
-      const int group = *reinterpret_cast<const volatile int*>(&hi->group), Tn = *reinterpret_cast<const volatile int*>(&hi->T);
-      const int gen = *reinterpret_cast<const volatile int*>(&hi->gen);
-      const uint32_t tg = sbase + sm.tags + static_cast<uint32_t>(hsl) * kNR * 4u;
-      Scan sc; sc.init(p.Gr);
-      int t = 1, t_stop = 0;
-      while (t <= Tn) {
-        // ---- which of the next NBK steps have arrived (lane k looks at step t + k)
-        uint32_t word = 0u;
-        int n;
-        {
-          ART_WATCH(wd, 5);
-          for (;;) {
-            bool ok = false;
-            if (lane < NBK && t + lane <= Tn) {
-              word = static_cast<uint32_t>(ld_volatile_s32(tg + static_cast<uint32_t>((t + lane - 1) % kNR) * 4u));
-              ok = (word >> 8) == static_cast<uint32_t>(t + lane);
-            }
-            const uint32_t bits = __ballot_sync(0xffffffffu, ok);
-            n = __ffs(~bits) - 1;
-            if (n > 0) break;
-            ART_WATCH_POLL(wd, hs, t);
-          }
-        }
-        // ---- pull the summaries: (m, l) of the owned step, P~V_t of every step at this lane's coordinates
-        float pv[NBK][CPL];
-        float m_own, l_own;
-        {
-          ART_WATCH(wd, 6);
-          for (;;) {
-            bool bad = false;
-            const uint32_t wk_own = __shfl_sync(0xffffffffu, word, own_k);
-            m_own = kNegInf; l_own = 0.f;
-            if (owner && own_k < n) {
-              const uint32_t base = mapa(sbase + sm.sums + (wk_own & 7u) * SUMB, (wk_own >> 4) & 15u);
-              uint32_t ml[2];
-              ld_cluster_vec<2>(base + (G * PW + 2 * h_lane) * 4u, ml);
-              const uint32_t par = (wk_own >> 3) & 1u;
-              bad = ((ml[0] ^ par) | (ml[1] ^ par)) & 1u;
-              m_own = __uint_as_float(ml[0]); l_own = __uint_as_float(ml[1]);
-              if (m_own <= -1e29f) m_own = kNegInf;
-            }
-#pragma unroll
-            for (int k = 0; k < NBK; ++k) {
-              const uint32_t wk = __shfl_sync(0xffffffffu, word, k);
-              if (k < n) {
-                const uint32_t base = mapa(sbase + sm.sums + (wk & 7u) * SUMB, (wk >> 4) & 15u);
-                uint32_t raw[CPL];
-                ld_cluster_vec<CPL>(base + static_cast<uint32_t>(lane * CPL) * 4u, raw);
-                const uint32_t par = (wk >> 3) & 1u;
-#pragma unroll
-                for (int j = 0; j < CPL; ++j) { bad |= ((raw[j] ^ par) & 1u) != 0u; pv[k][j] = __uint_as_float(raw[j]); }
-              } else {
-#pragma unroll
-                for (int j = 0; j < CPL; ++j) pv[k][j] = 0.f;
-              }
-            }
-            if (!__any_sync(0xffffffffu, bad)) break;         // a word of the slot's previous generation: look again
-            ART_WATCH_POLL(wd, hs, t);
-          }
-        }
-        const int fired = sc.chunk(n, lane, p.tau, p.phi, p.patience, m_own, l_own, pv);
-        const int t_last = fired >= 0 ? t + fired : t + n - 1;
-        const bool fin = fired >= 0 || t_last >= Tn;
-        if (fin) {
-          // t* is known: record it, let the last flusher recognise itself, THEN release the final progress word
-          t_stop = t_last;
-          if (lane == 0) {
-            p.stop_block[group] = t_stop;                    // t* (R9)
-            atom_add64_cluster_acqrel(hinfo_at(hs, H_DONE), static_cast<unsigned long long>(t_stop + 1) << 32);
-          }
-          __syncwarp();
-          if (lane < CL) st_cluster_release_s32(mapa(sbase + sm.ctrl + static_cast<uint32_t>(hs) * 4u, lane), ctrl_word(gen, fired >= 0, t_last));
-          break;
-        }
-        if (lane < CL) st_cluster_relaxed_s32(mapa(sbase + sm.ctrl + static_cast<uint32_t>(hs) * 4u, lane), ctrl_word(gen, false, t_last));
-        t += n;
-      }
-      (void)t_stop;
-      ++sg;
     }
   }
 
