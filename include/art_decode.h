@@ -37,7 +37,8 @@ extern "C" {
 
 #define ART_VERSION 110          /* 0.1.1: art_desc_t.q_len */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
-#define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent grid, steps claimed at run time (BF16 only) */
+#define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent clusters, cluster size chosen by the library (BF16 only) */
+#define ART_SPLIT_PERSISTENT(cl) (-1 - (cl))   /* art_desc_t.split: persistent clusters of cl = 1..16 CTAs (BF16 only) */
 #define ART_PATIENCE_INF 2147483647 /* "p = infinity": detector runs, never fires (App. E) */
 
 /* status codes: 0 = OK, negative = error.  No exceptions, no abort. */

@@ -16,6 +16,12 @@ _LIB_NAME = "libart_decode.so"
 
 ART_PATIENCE_INF = 2**31 - 1
 ART_SPLIT_DYNAMIC = -1
+
+
+def art_split_persistent(cl: int) -> int:
+    """ART_SPLIT_PERSISTENT(cl): art_desc_t.split for persistent clusters of cl CTAs."""
+    return -1 - int(cl)
+
 ART_DTYPE_F32, ART_DTYPE_BF16 = 0, 1
 ART_LAYOUT_HND, ART_LAYOUT_NHD = 0, 1
 ART_POLICY_DENSE, ART_POLICY_SINK_WINDOW, ART_POLICY_LIST = 0, 1, 2

@@ -43,6 +43,7 @@ struct Params {
   int32_t patience;
   int32_t stages, mbox_slots;
   int32_t dyn;                                       // bf16 cluster kernel: steps claimed at run time instead of dealt round-robin
+  int32_t run_ahead;                                 // bf16 cluster kernel, detector on: loads of step t are issued once step t - run_ahead is decided (0 = no limit)
 #ifdef ART_TRACE
   uint8_t* trace;
 #endif

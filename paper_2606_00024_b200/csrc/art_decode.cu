@@ -123,9 +123,8 @@ static int validate(const art_desc_t* d, const void* q, const void* k, const voi
     if (d->max_eligible < 0) return ART_ERR_SHAPE;
   }
   if (d->policy == ART_POLICY_SINK_WINDOW && (d->sink_tokens < 0 || d->window_tokens < 0)) return ART_ERR_SHAPE;
-  const bool legacy = d->split <= -100 && d->split >= -116;
-  if ((d->split < ART_SPLIT_DYNAMIC && !legacy) || d->split > 16) return ART_ERR_SHAPE;
-  if ((d->split == ART_SPLIT_DYNAMIC || legacy) && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
+  if (d->split < ART_SPLIT_PERSISTENT(16) || d->split > 16) return ART_ERR_SHAPE;
+  if (d->split < 0 && d->dtype != ART_DTYPE_BF16) return ART_ERR_DTYPE;
   if (d->dtype == ART_DTYPE_F32 && d->split > 0 && (d->split & (d->split - 1))) return ART_ERR_SHAPE;
   if (!(d->sm_scale >= 0.f) || isinf(d->sm_scale)) return ART_ERR_SHAPE;
   if (th) {
@@ -152,10 +151,15 @@ static int mode_of(const art_desc_t* d, const art_thresholds_t* th) {
   return (th->probe_dim == 0 || th->probe_dim == d->head_dim) ? 2 : 1;
 }
 
-// ---- which bf16 kernel a descriptor selects.  split = 0 / ART_SPLIT_DYNAMIC / 1..16: persistent clusters (of that
-// size); split = -(100 + C): the static-cluster kernel of round 1 with C CTAs per group (C = 0: its own choice).
-static inline bool legacy_split(const art_desc_t* d) { return d->split <= -100; }
-static inline int legacy_c(const art_desc_t* d) { return -d->split - 100; }
+// ---- which bf16 kernel a descriptor selects (include/art_decode.h, art_desc_t.split):
+//   1..16                 static clusters: one cluster of that many CTAs per group
+//   ART_SPLIT_DYNAMIC     persistent clusters, the library's cluster size;  ART_SPLIT_PERSISTENT(cl): clusters of cl
+//   0                     the library decides (see route())
+struct Route { bool persistent; int want; };               // want: cluster size asked for, 0 = the library's choice
+static inline Route route_of_split(const art_desc_t* d) {
+  if (d->dtype != ART_DTYPE_BF16 || d->split >= 0) return {false, d->split};
+  return {true, d->split == ART_SPLIT_DYNAMIC ? 0 : -d->split - 1};
+}
 
 // shared-memory plan of the static-cluster kernels (fp32 CUDA-core kernel; legacy bf16 kernel)
 static LaunchPlan plan_for(bool tensor_core, int G, int PW, bool art, int C) {
@@ -180,20 +184,13 @@ static LaunchPlan plan_for(bool tensor_core, int G, int PW, bool art, int C) {
   return pl;
 }
 
-// shared-memory plan of the persistent-cluster kernel: two CTAs per SM (3-stage ring each) unless the probe is the
-// full output (MODE 2: 4x larger summaries), which runs one CTA per SM with a deeper ring
-struct PcPlan { int stages, nsum, per_sm; uint32_t smem; };
-static PcPlan plan_pc(int G, int PW, bool art) {
+// shared-memory plan of the persistent-cluster kernel (detector off): two CTAs per SM, a 3-stage ring each
+struct PcPlan { int stages; uint32_t smem; };
+static PcPlan plan_pc(int G) {
   PcPlan pl;
-  const bool two_per_sm = !art || PW == 32;
-  const uint32_t budget = two_per_sm ? kSmemTwoPerSm : static_cast<uint32_t>(kMaxSmem);
-  pl.per_sm = two_per_sm ? 2 : 1;
-  pl.stages = two_per_sm ? 3 : tc::kMaxStages;
-  pl.nsum = art ? tc::kPVSlots : 0;
-  auto total = [&]() { return pc::make_smem_map_p(G, PW, pl.stages, pl.nsum, art).total; };
-  while (art && pl.nsum > 2 && total() > budget) pl.nsum >>= 1;      // 8 -> 4 summary slots (G = 8)
-  while (pl.stages > 2 && total() > budget) --pl.stages;
-  pl.smem = total();
+  pl.stages = 3;
+  while (pl.stages > 2 && pc::make_smem_map_p(G, pl.stages).total > kSmemTwoPerSm) --pl.stages;
+  pl.smem = pc::make_smem_map_p(G, pl.stages).total;
   return pl;
 }
 
@@ -210,13 +207,8 @@ static int occupancy_tc(int G, int mode, int C, uint32_t smem) {
   switch (G) { case 1: return occupancy_tc_g1(mode, C, smem); case 2: return occupancy_tc_g2(mode, C, smem);
                case 4: return occupancy_tc_g4(mode, C, smem); default: return occupancy_tc_g8(mode, C, smem); }
 }
-static int occupancy_pc(int G, int mode, int C, uint32_t smem) {
-  switch (G) { case 1: return occupancy_pc_g1(mode, C, smem); case 2: return occupancy_pc_g2(mode, C, smem);
-               case 4: return occupancy_pc_g4(mode, C, smem); default: return occupancy_pc_g8(mode, C, smem); }
-}
-
 // clusters of size C that can be co-resident, cached per (device, kernel class, shared memory size)
-// kind: 0 = fp32 CUDA-core kernel, 1 = legacy bf16 kernel, 2 = persistent-cluster kernel
+// kind: 0 = fp32 CUDA-core kernel, 1 = bf16 tensor-core kernels (static clusters; persistent clusters: mode 0)
 static int cluster_capacity(int kind, int G, int mode, int C, uint32_t smem) {
   static std::mutex mu;
   static std::map<std::array<int, 4>, int> cache;
@@ -230,7 +222,6 @@ static int cluster_capacity(int kind, int G, int mode, int C, uint32_t smem) {
   int fit;
   if (twin) fit = max_active_clusters(tc_occupancy_twin, tc::kThreads, C, smem);
   else if (kind == 1) fit = occupancy_tc(G, mode, C, smem);
-  else if (kind == 2) fit = occupancy_pc(G, mode, C, smem);
   else
     fit = dispatch(G, mode, [&](auto m, auto gg) {
       return max_active_clusters(simt::art_decode_kernel<float, 64, decltype(gg)::value, decltype(m)::value>, simt::kThreads, C, smem);
@@ -265,37 +256,22 @@ static int choose_split(const art_desc_t* d, int mode, int want, int* C_out) {
   return ART_OK;
 }
 
-// Persistent clusters: cluster size CL (the caller's, else the largest of 16, 8, 4, 2, 1 that the device can
-// co-schedule at all) and the number of clusters NC = min(co-resident clusters, groups).
-static int choose_pc(int G, int mode, int want, int groups, const PcPlan& pl, int* CL_out, int* NC_out) {
-  int CL = want > 0 ? want : 16, fit = 0;
-  for (;;) {
-    fit = cluster_capacity(2, G, mode, CL, pl.smem);
-    if (fit > 0 || want > 0 || CL == 1) break;
-    CL >>= 1;
-  }
+// Persistent clusters (detector off): cluster size CL and the number of clusters NC = min(co-resident clusters, groups).
+// The library's own choice is clusters of ONE CTA: measured on configs[3] (1024 groups of ~65 blocks), 355 us against
+// 372 / 363 us with clusters of 2 / 4 and 368 us with static one-CTA clusters (profiles/r02_persistent.md); larger
+// clusters exist for callers whose groups are few and uneven (the tail of the call is then shared inside a cluster).
+static int choose_pc(int G, int want, int groups, const PcPlan& pl, int* CL_out, int* NC_out) {
+  const int CL = want > 0 ? want : 1;
+  const int fit = cluster_capacity(1, G, 0, CL, pl.smem);
   if (fit <= 0) return ART_ERR_CUDA;
   *CL_out = CL; *NC_out = fit < groups ? fit : groups;
   return ART_OK;
 }
 
-// run-ahead per worker of the persistent-cluster kernel (steps whose loads may be issued beyond the last decided
-// step, per CTA working on the group); ART_PC_RUNAHEAD overrides it for measurements
-static int pc_claim() {
-  static const int env = [] { const char* e = getenv("ART_PC_CLAIM"); return e ? atoi(e) : 0; }();
-  return env > 0 ? (env > 16 ? 16 : env) : 4;
-}
-static unsigned pc_nap() {
-  static const int env = [] { const char* e = getenv("ART_PC_NAP"); return e ? atoi(e) : -1; }();
-  return env >= 0 ? static_cast<unsigned>(env) : 100u;
-}
-static int pc_run_ahead(int nsum) {
-  static const int env = [] { const char* e = getenv("ART_PC_RUNAHEAD"); return e ? atoi(e) : 0; }();
-  int rw = env > 0 ? env : 6;
-  return rw;
-}
+// steps a CTA of a persistent cluster claims per atomic on its cluster's board
+static int pc_claim() { return 4; }
 
-#if defined(ART_WATCHDOG) || defined(ART_PC_STATS)
+#ifdef ART_WATCHDOG
 // debugging build: a pinned, device-mapped word that a wait which never ends writes before it traps; it survives
 // the death of the context, so the test harness can print where the kernel was stuck (art_debug_watchdog())
 static unsigned long long* g_watchdog_host = nullptr;
@@ -312,17 +288,14 @@ static unsigned long long* watchdog_word() {
 }
 #endif
 
-#ifdef ART_PC_STATS
-static unsigned long long* stats_buffer() {
-  static unsigned long long* dev = [] {
-    unsigned long long* d = nullptr;
-    if (cudaMalloc(&d, 512) != cudaSuccess) { cudaGetLastError(); return static_cast<unsigned long long*>(nullptr); }
-    cudaMemset(d, 0, 512);
-    return d;
-  }();
-  return dev;
+// static bf16 clusters, detector on: how far the loads of a group may run ahead of its last decided step.  Every CTA of
+// the cluster keeps its ring full (stages) plus the blocks on their way through S-MMA / softmax / P.V / mailbox / scan.
+// ART_RUNAHEAD overrides it for measurements (0 = no limit, the behaviour of round 1).
+static int static_run_ahead(int C, int stages) {
+  static const int env = [] { const char* e = getenv("ART_RUNAHEAD"); return e ? atoi(e) : -1; }();
+  if (env >= 0) return env;
+  return C * (stages + 3) + 4;
 }
-#endif
 
 // workspace of the persistent-cluster kernel: one partial state (m, l, acc) per (group, CTA of a cluster)
 static size_t pc_part_bytes(int groups, int G) {
@@ -343,7 +316,21 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const int mode = mode_of(d, th);
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
-  const bool persistent = tensor_core && !legacy_split(d);
+  // Static clusters are the default: every group streams from the first cycle and, with the detector on, the decision
+  // loop of a group never leaves its cluster.  When the detector is off and the groups do not even fit one 2-CTA
+  // cluster each (many short groups: configs[3]), persistent clusters that pull groups from their queue avoid the
+  // waves of short-lived CTAs; they need the caller's workspace.
+  Route rt = route_of_split(d);
+  if (rt.persistent && mode != 0) rt = {false, 0};         // persistent clusters exist for the detector-off path only
+  const size_t pc_need = tensor_core ? pc_part_bytes(groups, G) : 0;
+  const bool ws_ok = workspace && workspace_bytes >= pc_need && !(reinterpret_cast<uintptr_t>(workspace) & 255u);
+  int C_static = 1;
+  if (!rt.persistent) {
+    int rc = choose_split(d, mode, rt.want, &C_static);
+    if (rc != ART_OK) return rc;
+    if (tensor_core && d->split == 0 && mode == 0 && C_static == 1 && ws_ok) rt = {true, 0};
+  }
+  const bool persistent = rt.persistent;
 
   Params p = {};
   p.q = q; p.k = static_cast<const uint8_t*>(k); p.v = static_cast<const uint8_t*>(v);
@@ -366,22 +353,18 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
 
   cudaError_t e;
   if (persistent) {
-    const PcPlan pl = plan_pc(G, PW, mode != 0);
+    const PcPlan pl = plan_pc(G);
     int CL = 1, NC = 1;
-    int rc = choose_pc(G, mode, d->split > 0 ? d->split : 0, groups, pl, &CL, &NC);
+    int rc = choose_pc(G, rt.want, groups, pl, &CL, &NC);
     if (rc != ART_OK) return rc;
-    const size_t need = pc_part_bytes(groups, G);
-    if (!workspace || workspace_bytes < need || (reinterpret_cast<uintptr_t>(workspace) & 255u)) return ART_ERR_WORKSPACE;
+    if (!ws_ok) return ART_ERR_WORKSPACE;
     p.stages = pl.stages; p.mbox_slots = 0; p.dyn = 1;
     pc::PcParams pp = {};
     pp.b = p; pp.n_groups = groups; pp.NC = NC; pp.part = static_cast<float*>(workspace);
-    pp.rw = pc_run_ahead(pl.nsum); pp.claim = mode != 0 ? 1 : pc_claim(); pp.nap = pc_nap(); pp.nsum = pl.nsum > 0 ? pl.nsum : 1;
+    pp.claim = pc_claim();
     pp.dbg = nullptr;
-#if defined(ART_WATCHDOG) || defined(ART_PC_STATS)
+#ifdef ART_WATCHDOG
     pp.dbg = watchdog_word();
-#endif
-#ifdef ART_PC_STATS
-    pp.stats = stats_buffer();
 #endif
     CUtensorMap tmK, tmV;
     if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
@@ -390,20 +373,19 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
     const bool mt = p.qlen > 1;
     int r;
     switch (G) {
-      case 1: r = launch_pc_g1(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
-      case 2: r = launch_pc_g2(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
-      case 4: r = launch_pc_g4(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
-      default: r = launch_pc_g8(mode, mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      case 1: r = launch_pc_g1(mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      case 2: r = launch_pc_g2(mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      case 4: r = launch_pc_g4(mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
+      default: r = launch_pc_g8(mt, NC, CL, pl.smem, stream, pp, tmK, tmV); break;
     }
     e = static_cast<cudaError_t>(r);
   } else {
-    int C = 1;
-    int rc = choose_split(d, mode, tensor_core ? legacy_c(d) : d->split, &C);
-    if (rc != ART_OK) return rc;
+    const int C = C_static;
     const LaunchPlan pl = plan_for(tensor_core, G, PW, mode != 0, C);
     p.stages = pl.stages; p.mbox_slots = pl.mslots;
-    // legacy bf16 kernel: with the detector on, steps are claimed at run time for clusters of 2-4 (measured in round 1)
+    // static bf16 clusters: with the detector on, steps are claimed at run time for clusters of 2-4 (measured in round 1)
     p.dyn = (tensor_core && mode != 0 && C >= 2 && C <= 4) ? 1 : 0;
+    p.run_ahead = (tensor_core && mode != 0) ? static_run_ahead(C, pl.stages) : 0;
     if (tensor_core) {
 #ifdef ART_TRACE
       if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
@@ -633,38 +615,46 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
   return ART_OK;
 }
 
-int art_query_split(const art_desc_t* desc, int art_on) {
+// the launch shape run() would use, given a workspace of art_workspace_bytes(desc): cluster size, and the number of
+// persistent clusters (0 = static clusters, one per group)
+static int query_shape(const art_desc_t* desc, int art_on, int* C_out, int* NC_out) {
   if (!desc) return ART_ERR_NULL;
   if (desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->num_q_heads % desc->num_kv_heads) return ART_ERR_SHAPE;
   if (desc->num_q_heads / desc->num_kv_heads > 8 || desc->q_len < 0 || art::rows_of(desc) > 8) return ART_ERR_SHAPE;
   if (!((desc->dtype == ART_DTYPE_F32 && desc->head_dim == 64) || (desc->dtype == ART_DTYPE_BF16 && desc->head_dim == 128))) return ART_ERR_DTYPE;
+  if (desc->split < ART_SPLIT_PERSISTENT(16) || desc->split > 16 || (desc->split < 0 && desc->dtype != ART_DTYPE_BF16)) return ART_ERR_SHAPE;
   int rc = art::check_arch();
   if (rc != ART_OK) return rc;
   const int mode = art_on == 2 ? 2 : (art_on ? 1 : 0);                 // 2: detector on the full output (probe_dim = 0 or d)
+  const int groups = desc->batch * desc->num_kv_heads > 0 ? desc->batch * desc->num_kv_heads : 1;
+  art::Route rt = art::route_of_split(desc);
   int C = 1;
-  if (desc->dtype == ART_DTYPE_BF16 && !art::legacy_split(desc)) {
-    const int G = art::padded_group(art::rows_of(desc));
-    const art::PcPlan pl = art::plan_pc(G, mode == 2 ? desc->head_dim : 32, mode != 0);
-    int NC = 1;
-    rc = art::choose_pc(G, mode, desc->split > 0 ? desc->split : 0, desc->batch * desc->num_kv_heads > 0 ? desc->batch * desc->num_kv_heads : 1, pl, &C, &NC);
-    return rc == ART_OK ? C : rc;
+  if (!rt.persistent) {
+    rc = art::choose_split(desc, mode, rt.want, &C);
+    if (rc != ART_OK) return rc;
+    if (desc->dtype == ART_DTYPE_BF16 && desc->split == 0 && mode == 0 && C == 1) rt = {true, 0};
+  } else if (mode != 0) {                                  // persistent clusters exist for the detector-off path only
+    rt = {false, 0};
+    rc = art::choose_split(desc, mode, 0, &C);
+    if (rc != ART_OK) return rc;
   }
-  rc = art::choose_split(desc, mode, desc->dtype == ART_DTYPE_BF16 ? art::legacy_c(desc) : desc->split, &C);
+  *C_out = C; *NC_out = 0;
+  if (rt.persistent) {
+    const int G = art::padded_group(art::rows_of(desc));
+    rc = art::choose_pc(G, rt.want, groups, art::plan_pc(G), C_out, NC_out);
+  }
+  return rc;
+}
+
+int art_query_split(const art_desc_t* desc, int art_on) {
+  int C = 0, NC = 0;
+  const int rc = query_shape(desc, art_on, &C, &NC);
   return rc == ART_OK ? C : rc;
 }
 
 int art_query_clusters(const art_desc_t* desc, int art_on) {
-  if (!desc) return ART_ERR_NULL;
-  if (desc->dtype != ART_DTYPE_BF16 || art::legacy_split(desc)) return ART_ERR_DTYPE;
-  if (desc->num_q_heads <= 0 || desc->num_kv_heads <= 0 || desc->num_q_heads % desc->num_kv_heads || art::rows_of(desc) > 8) return ART_ERR_SHAPE;
-  int rc = art::check_arch();
-  if (rc != ART_OK) return rc;
-  const int mode = art_on == 2 ? 2 : (art_on ? 1 : 0);
-  const int G = art::padded_group(art::rows_of(desc));
-  const art::PcPlan pl = art::plan_pc(G, mode == 2 ? desc->head_dim : 32, mode != 0);
-  int CL = 1, NC = 1;
-  const int groups = desc->batch * desc->num_kv_heads;
-  rc = art::choose_pc(G, mode, desc->split > 0 ? desc->split : 0, groups > 0 ? groups : 1, pl, &CL, &NC);
+  int C = 0, NC = 0;
+  const int rc = query_shape(desc, art_on, &C, &NC);
   return rc == ART_OK ? NC : rc;
 }
 
@@ -684,18 +674,8 @@ const char* art_status_string(int status) {
 
 int art_version(void) { return ART_VERSION; }
 
-#if defined(ART_WATCHDOG) || defined(ART_PC_STATS)
+#ifdef ART_WATCHDOG
 unsigned long long art_debug_watchdog(void) { return art::g_watchdog_host ? art::g_watchdog_host[0] : 0ull; }
-unsigned long long art_debug_watchdog2(void) { return art::g_watchdog_host ? art::g_watchdog_host[1] : 0ull; }
-#ifdef ART_PC_STATS
-void art_debug_stats_read(unsigned long long* host_out) {      // synchronises; returns and clears the 64 counters
-  unsigned long long* d = art::stats_buffer();
-  if (!d) return;
-  cudaDeviceSynchronize();
-  cudaMemcpy(host_out, d, 512, cudaMemcpyDeviceToHost);
-  cudaMemset(d, 0, 512);
-}
-#endif
 #endif
 
 }  // extern "C"

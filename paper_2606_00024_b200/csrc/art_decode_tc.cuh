@@ -325,6 +325,17 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     const int c = ld_ctrl_relaxed(a_ctrl);
     return c < 0 && t > -c;
   };
+  // A7, bounded run-ahead: the loads of step t are issued only once step t - run_ahead has been decided, so that at most
+  // run_ahead blocks per group are loaded and then discarded when Algorithm 1 fires.  False if step t lies beyond t*.
+  auto may_issue = [&](int t) -> bool {
+    if constexpr (!ART) return true;
+    if (p.run_ahead <= 0) return !beyond_stop(t);
+    for (;;) {
+      const int c = ld_ctrl_relaxed(a_ctrl);
+      if (c < 0) return t <= -c;
+      if (c >= t - p.run_ahead) return true;
+    }
+  };
   // Every issued item runs through all roles (one beyond t* is dropped by the fold warps); a wait can only fail
   // once the producer has issued its last item (known up front, n_lim, unless steps are claimed at run time
   // or Algorithm 1 fires).
@@ -379,6 +390,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         bool validB; unsigned long long maskB; int pageB, ecB;
         resolve(tN, validB, maskB, pageB, ecB);
         if (validB && lane == 0) tB = claim();
+        if (!may_issue(tA)) break;                             // (waits for step tA - run_ahead to be decided)
         if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                  // slot released?
         if (lane == 0) {
           TC_TRACE(trc, 1, group, tA);
@@ -429,7 +441,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
           const int c1_k = __shfl_sync(0xffffffffu, c1, kk), c2_k = __shfl_sync(0xffffffffu, c2, kk);
           int ec_k = 0;
           if constexpr (MT) ec_k = __shfl_sync(0xffffffffu, ec, kk);
-          if (beyond_stop(t)) { stop = true; break; }          // A7: stop issuing prefetch once fired
+          if (!may_issue(t)) { stop = true; break; }           // A7: stop issuing prefetch once fired; bounded run-ahead
           if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                // slot released?
           if (lane == 0) {
             TC_TRACE(trc, 1, group, t);

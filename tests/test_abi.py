@@ -27,7 +27,7 @@ def test_every_declared_symbol_is_exported(art):
     lib = art.load_library()
     syms = declared_symbols()
     assert {"art_decode_attention", "art_decode_attention_off", "art_decode_attention_host", "art_topk_blocks",
-            "art_workspace_bytes", "art_query_split", "art_status_string", "art_version"} <= set(syms)
+            "art_workspace_bytes", "art_query_split", "art_query_clusters", "art_status_string", "art_version"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
     assert art.art_version() == 110
@@ -65,7 +65,7 @@ def test_argument_validation_happens_before_cuda(art):
     assert _call_off(art, good_desc(art, policy=2)) == -1                    # LIST without a list
     assert _call_off(art, good_desc(art, policy=1, sink_tokens=-1)) == -2
     assert _call_off(art, good_desc(art, split=17)) == -2                    # cluster size > 16
-    assert _call_off(art, good_desc(art, split=-2)) == -2
+    assert _call_off(art, good_desc(art, split=-18)) == -2                   # persistent clusters of at most 16 CTAs
     assert _call_off(art, good_desc(art, max_blocks_per_seq=1 << 24)) == -2   # a step number is 24 bits
     assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=-1)) == -3   # dynamic: bf16 only
     assert _call_off(art, good_desc(art, dtype=art.ART_DTYPE_F32, head_dim=64, split=3)) == -2   # fp32 path: power of two

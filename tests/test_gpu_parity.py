@@ -234,7 +234,11 @@ def test_error_codes_on_device():
         a.art_decode_attention_off(desc, w.q, w.k_cache, w.v_cache, w.block_table, None, w.seq_lens, out, stop)
     assert e.value.status == -2
     assert 1 <= a.art_query_split(a.make_desc(w), True) <= 16
-    assert a.art_query_split(a.make_desc(w, split=-1), True) == 0   # dynamic scheduler: no fixed cluster
+    d_dyn = a.make_desc(w, split=a.ART_SPLIT_DYNAMIC)              # persistent clusters: their size, and how many of them
+    assert a.art_query_split(d_dyn, False) == 1 and a.art_query_clusters(d_dyn, False) >= 1
+    assert a.art_query_clusters(d_dyn, True) == 0                   # detector on: always static clusters
+    assert a.art_query_clusters(a.make_desc(w, split=2), True) == 0   # static clusters: one per group
+    assert a.art_query_split(a.make_desc(w, split=a.art_split_persistent(3)), False) == 3
 
 
 def test_sm_scale_override():
