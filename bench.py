@@ -154,6 +154,17 @@ def reduce_over_ranks(ms: float, toks: float, device="cpu"):
     return float(t), float(tk)
 
 
+def read_only_ceiling(art, w, steps: int, warmup: int) -> float:
+    """GB/s of a read-only stream over this workload's K and V caches (art_hbm_read_probe: 32 KiB TMA copies, 3-stage
+    ring, two CTAs per SM, no compute); both buffers are larger than L2 and are streamed alternately."""
+    def fn():
+        art.art_hbm_read_probe(w.k_cache)
+        art.art_hbm_read_probe(w.v_cache)
+    ms = time_loop(fn, steps, warmup)
+    nbytes = sum((t.numel() * t.element_size()) // BLOCK_BYTES * BLOCK_BYTES for t in (w.k_cache, w.v_cache))
+    return nbytes * steps / (ms * 1e-3) / 1e9
+
+
 def make_runner(art, w, *, art_on: bool, split: int = 0, **th):
     """Pre-marshalled call (descriptors and outputs allocated once); returns (fn, out, stop, loaded)."""
     import torch
@@ -202,28 +213,61 @@ def measure(art, w, steps, warmup, barrier=None, *, art_on=True, split=0, **th):
             "gbs_loaded": ld * BLOCK_BYTES / (us * 1e-6) / 1e9, "ms_total": ms}
 
 
-def oracle_sample(w, n_groups: int, art_on: bool = True):
-    """The CPU oracle, as it stands, on a bounded sample of groups of workload w (single BLAS thread).
-    Returns (seconds, sequence-level KV tokens covered, threads)."""
+def _oracle_groups(args):
+    """Worker (own process): the oracle on the groups of one small carved-out workload, one BLAS thread."""
+    mini, art_on = args
     sys.path.insert(0, os.path.join(ROOT, "tests"))
-    from helpers import extract_groups, run_oracle       # imports oracle/: cpu_baseline leg only
-    import numpy as np
-    rng = np.random.default_rng(0)
-    B, Hkv = w.batch, w.num_kv_heads
-    groups = [(int(rng.integers(B)), int(rng.integers(Hkv))) for _ in range(n_groups)]
-    mini = extract_groups(w, groups)
+    from helpers import run_oracle                       # imports oracle/: cpu_baseline leg only
     try:
         from threadpoolctl import threadpool_limits
         ctx = threadpool_limits(limits=1)
     except Exception:
         import contextlib
         ctx = contextlib.nullcontext()
-    tokens_all = eligible_tokens(mini)                   # mini has Hkv = 1: per-group tokens
     with ctx:
         t0 = time.perf_counter()
         run_oracle(mini, art=art_on)
-        dt = time.perf_counter() - t0
+        return time.perf_counter() - t0
+
+
+def oracle_sample(w, n_groups: int, art_on: bool = True):
+    """The CPU oracle, as it stands, on a bounded sample of groups of workload w (single BLAS thread).
+    Returns (seconds, sequence-level KV tokens covered, threads)."""
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import extract_groups                   # pure data movement
+    import numpy as np
+    rng = np.random.default_rng(0)
+    B, Hkv = w.batch, w.num_kv_heads
+    groups = [(int(rng.integers(B)), int(rng.integers(Hkv))) for _ in range(n_groups)]
+    mini = extract_groups(w, groups)
+    tokens_all = eligible_tokens(mini)                   # mini has Hkv = 1: per-group tokens
+    dt = _oracle_groups((mini, art_on))
     return dt, tokens_all / Hkv, 1
+
+
+def oracle_sample_all_cores(w, groups_per_core: int = 2, art_on: bool = True):
+    """The same oracle, the same way, with the sampled groups spread over every host core (one process per core, one
+    BLAS thread each).  Returns (wall seconds of the parallel section, sequence-level KV tokens covered, processes)."""
+    import multiprocessing as mp
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import extract_groups
+    import numpy as np
+    n = os.cpu_count() or 1
+    rng = np.random.default_rng(1)
+    B, Hkv = w.batch, w.num_kv_heads
+    jobs, toks = [], 0.0
+    for _ in range(n):
+        groups = [(int(rng.integers(B)), int(rng.integers(Hkv))) for _ in range(groups_per_core)]
+        mini = extract_groups(w, groups)
+        toks += eligible_tokens(mini) / Hkv
+        jobs.append((mini, art_on))
+    os.environ["PYTHONPATH"] = os.pathsep.join([ROOT, os.path.join(ROOT, "tests"), os.environ.get("PYTHONPATH", "")])
+    with mp.get_context("spawn").Pool(n) as pool:
+        pool.map(_oracle_groups, [(jobs[0][0], art_on)] * n)     # warm-up: imports, page-in (untimed)
+        t0 = time.perf_counter()
+        pool.map(_oracle_groups, jobs, chunksize=1)
+        dt = time.perf_counter() - t0
+    return dt, toks, n
 
 
 def run_reference(args, rank, world):
@@ -251,6 +295,56 @@ def run_reference(args, rank, world):
     print(json.dumps(line), flush=True)
 
 
+def sampled_parity(art, w, art_on: bool, n_groups: int, split: int = 0):
+    """GPU vs oracle on a few sampled groups of a full-size workload (tests/parity.py): stop-block mismatches on
+    non-fragile / fragile groups, fragile groups, max relative output error."""
+    import numpy as np
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import extract_groups
+    from parity import compare
+    rng = np.random.default_rng(5)
+    groups = sorted({(int(rng.integers(w.batch)), int(rng.integers(w.num_kv_heads))) for _ in range(n_groups)})
+    out, stop, _ = art.run_workload(w, art=art_on, split=split)
+    torch.cuda.synchronize()
+    G = w.group_size
+    mini = extract_groups(w, groups)
+    o_g = torch.stack([out[b, g * G:(g + 1) * G] for (b, g) in groups])
+    s_g = torch.stack([stop[b, g:g + 1] for (b, g) in groups])
+    rep = compare(mini, o_g, s_g, art=art_on)
+    return {"groups": rep.groups, "stop_mismatch_nonfragile": rep.stop_mismatch_nonfragile,
+            "stop_mismatch_fragile": rep.stop_mismatch_fragile, "fragile_groups": rep.fragile_groups,
+            "fragile_unreachable": rep.fragile_unreachable, "max_rel_err": rep.max_rel_err}
+
+
+def needle_report(art, w):
+    """configs[4] (the NIAH failure mode of PAPER.md:216-236 Table 2 in synthetic form): per sequence,
+    did Algorithm 1 fire, t* against the step at which the needle block is visited (dense order: step T - n_b), and the
+    truncation error |out_on - out_off|_inf / |out_off|_inf of the ORACLE for one group of the sequence, next to the
+    GPU's stop block for that group."""
+    import numpy as np
+    import torch
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    from helpers import extract_groups, run_oracle
+    out, stop, _ = art.run_workload(w, art=True)
+    torch.cuda.synchronize()
+    rows = []
+    for b in range(w.batch):
+        T = (int(w.seq_lens[b]) + 63) // 64
+        nb = int(w.notes["needle_block"][b])
+        g = b % w.num_kv_heads
+        mini = extract_groups(w, [(b, g)])
+        _, _, res = run_oracle(mini, art=True)
+        r = res[(0, 0)]
+        err = float(np.abs(r.out_on - r.out_off).max(axis=-1).max() / np.abs(r.out_off).max())
+        st = stop[b].cpu().numpy()
+        rows.append({"seq": b, "T": T, "needle_block": nb, "needle_step": T - nb, "gpu_t_star_min": int(st.min()), "gpu_t_star_max": int(st.max()),
+                     "groups_that_stop_before_the_needle": int((st < T - nb).sum()), "oracle_group": [b, g],
+                     "oracle_t_star": int(r.stop_block), "gpu_t_star_same_group": int(st[g]), "oracle_fired": bool(r.fired),
+                     "oracle_rel_trunc_err": err})
+    return rows
+
+
 def run_report(args):
     """All five configs (+ variants R / 0c), ART-on / ART-off / p = inf; one JSON line per row."""
     import torch
@@ -259,16 +353,23 @@ def run_report(args):
     peak, which = peaks()
     rows = [(0, "a", ""), (0, "a", "c"), (1, "a", ""), (1, "a", "R"), (2, "a", ""), (2, "a", "R"),
             (3, "a", ""), (3, "a", "R"), (3, "b", ""), (3, "b", "R"), (4, "a", ""), (4, "a", "R")]
+    ceiling = None
     for index, sub, variant in rows:
         w = gen.config(index, sub=sub, variant=variant, device="cuda")
         torch.cuda.synchronize()
+        if ceiling is None and w.dtype == torch.bfloat16:
+            ceiling = read_only_ceiling(art, w, args.steps, args.warmup)
         toks = eligible_tokens(w)
         sp = args.split if w.dtype == torch.bfloat16 else 0
         off = measure(art, w, args.steps, args.warmup, art_on=False, split=sp)
         on = measure(art, w, args.steps, args.warmup, art_on=True, split=sp)
         pinf = measure(art, w, args.steps, args.warmup, art_on=True, split=sp, patience=art.ART_PATIENCE_INF)
         total_blocks = off["blocks_processed"]
-        row = {"workload": w.name, "groups": w.batch * w.num_kv_heads, "split_on": art.art_query_split(art.make_desc(w, split=sp), True),
+        groups = w.batch * w.num_kv_heads
+        d_off, d_on = art.make_desc(w, split=sp), art.make_desc(w, split=sp)
+        row = {"workload": w.name, "groups": groups,
+               "split_on": art.art_query_split(d_on, True), "split_off": art.art_query_split(d_off, False),
+               "persistent_clusters_off": art.art_query_clusters(d_off, False) if w.dtype == torch.bfloat16 else 0,
                "eligible_tokens": toks, "blocks_total": total_blocks,
                "off_us": round(off["us_per_step"], 2), "off_gbs": round(off["gbs_processed"], 1),
                "off_frac_of_peak": round(off["gbs_processed"] / peak, 4),
@@ -277,10 +378,21 @@ def run_report(args):
                "on_gbs_processed": round(on["gbs_processed"], 1),
                "skipped_frac": round(1 - on["blocks_processed"] / max(total_blocks, 1), 4),
                "loaded_frac": round(on["blocks_loaded"] / max(total_blocks, 1), 4),
+               "loaded_over_processed": round(on["blocks_loaded"] / max(on["blocks_processed"], 1), 4),
+               "discarded_blocks_per_group": round((on["blocks_loaded"] - on["blocks_processed"]) / groups, 2),
                "speedup_on_vs_off": round(off["us_per_step"] / on["us_per_step"], 4),
                "pinf_overhead": round(pinf["us_per_step"] / off["us_per_step"] - 1, 4),
                "kv_tok_s_on": toks / (on["us_per_step"] * 1e-6), "kv_tok_s_off": toks / (off["us_per_step"] * 1e-6),
-               "peak_gbs": peak, "peak_kind": which}
+               "kv_tok_s_on_x_hkv": toks * w.num_kv_heads / (on["us_per_step"] * 1e-6),
+               "kv_tok_s_on_physical": on["blocks_processed"] * 64 / (on["us_per_step"] * 1e-6),
+               "peak_gbs": peak, "peak_kind": which,
+               "read_only_ceiling_gbs": None if ceiling is None else round(ceiling, 1),
+               "off_frac_of_read_only_ceiling": None if ceiling is None else round(off["gbs_processed"] / ceiling, 4)}
+        if not args.no_parity:
+            row["parity_on"] = sampled_parity(art, w, True, 4, sp)
+            row["parity_off"] = sampled_parity(art, w, False, 2, sp)
+            if index == 4:
+                row["needle"] = needle_report(art, w)
         print(json.dumps(row), flush=True)
         del w
         torch.cuda.empty_cache()
@@ -375,6 +487,7 @@ def main():
     ap.add_argument("--policy", action="store_true", help="time art_topk_blocks (SURVEY 8(f).3)")
     ap.add_argument("--study", action="store_true", help="probe-vs-full, ablation and sensitivity sweeps (SURVEY 8(f))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-parity", action="store_true", help="--report without the oracle columns (timing only)")
     ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
                     help="time ONLY this arm of one config (short command for ncu captures; prints a small JSON line)")
@@ -480,9 +593,9 @@ def main():
     pinf = measure(art, w, args.steps, args.warmup, barrier, art_on=True, patience=art.ART_PATIENCE_INF)
     r_off = measure(art, wR, args.steps, args.warmup, barrier, art_on=False)
     r_on = measure(art, wR, args.steps, args.warmup, barrier, art_on=True)
-    # the dynamically scheduled kernel (desc.split = ART_SPLIT_DYNAMIC), same two workloads
-    d_on = measure(art, w, args.steps, args.warmup, barrier, art_on=True, split=art.ART_SPLIT_DYNAMIC)
-    dr_on = measure(art, wR, args.steps, args.warmup, barrier, art_on=True, split=art.ART_SPLIT_DYNAMIC)
+    # the read-only streaming ceiling of this box, measured here and now: the K and V caches of the
+    # workload (512 MiB each, both larger than L2) streamed alternately by art_hbm_read_probe
+    ceiling_gbs = read_only_ceiling(art, w, args.steps, args.warmup)
 
     if rank == 0:
         us = ms / args.steps * 1e3             # this rank's own kernel time per launch
@@ -502,8 +615,9 @@ def main():
             "gpu_launches": args.steps,
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "traffic": traffic, "peak_kind": which,
-                         "kernel": "art_decode_kernel<bf16,128,G=4,ART on>",
-                         "bytes_per_launch": ld * BLOCK_BYTES, "frac_of_nominal_8TBs": achieved / 8000.0},
+                         "kernel": "art::tc::art_decode_tc_kernel<4, 1, false>",
+                         "bytes_per_launch": ld * BLOCK_BYTES, "frac_of_nominal_8TBs": achieved / 8000.0,
+                         "read_only_ceiling_gbs": ceiling_gbs, "frac_of_read_only_ceiling": achieved / ceiling_gbs},
             "art": {"on_us_per_step": us, "off_us_per_step": off["us_per_step"],
                     "off_gbs": off["gbs_processed"], "off_frac_of_peak": off["gbs_processed"] / peak,
                     "pinf_overhead": pinf["us_per_step"] / off["us_per_step"] - 1.0,
@@ -513,16 +627,21 @@ def main():
                                   "speedup_on_vs_off": r_off["us_per_step"] / r_on["us_per_step"],
                                   "skipped_frac": 1.0 - r_on["blocks_processed"] / max(r_off["blocks_processed"], 1),
                                   "loaded_frac": r_on["blocks_loaded"] / max(r_off["blocks_processed"], 1),
-                                  "on_gbs_loaded": r_on["gbs_loaded"], "on_frac_of_peak_loaded": r_on["gbs_loaded"] / peak},
-                    "dynamic_scheduler": {"on_us_per_step": d_on["us_per_step"],
-                                          "variant_R_on_us_per_step": dr_on["us_per_step"],
-                                          "variant_R_speedup_on_vs_off": r_off["us_per_step"] / dr_on["us_per_step"],
-                                          "variant_R_loaded_frac": dr_on["blocks_loaded"] / max(r_off["blocks_processed"], 1)}},
+                                  "on_gbs_loaded": r_on["gbs_loaded"], "on_frac_of_peak_loaded": r_on["gbs_loaded"] / peak,
+                                  "loaded_over_processed": r_on["blocks_loaded"] / max(r_on["blocks_processed"], 1),
+                                  "discarded_blocks_per_group": (r_on["blocks_loaded"] - r_on["blocks_processed"]) / (wR.batch * wR.num_kv_heads)},
+                    "off_frac_of_read_only_ceiling": off["gbs_processed"] / ceiling_gbs},
         }
+        line["kv_tok_s_x_hkv"] = value * w.num_kv_heads       # every KV head streams its own copy of the context
+        line["kv_tok_s_physical"] = processed * 64 / (us * 1e-6)   # tokens of the blocks actually visited, all heads, this rank
         if world == 1 and not args.no_cpu_baseline:
             dt, ctoks, cores = oracle_sample(w, 16)
+            dta, ctoka, ncore = oracle_sample_all_cores(w, 2)
             line["cpu_baseline"] = {"value": ctoks / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                    "sample": "16 of 64 (sequence, KV-head) groups of configs[1], one pass, ART on"}
+                                    "sample": "16 of 64 (sequence, KV-head) groups of configs[1], one pass, ART on",
+                                    "all_cores": {"value": ctoka / dta, "unit": UNIT, "cores": ncore,
+                                                  "sample": "2 groups per core, one process per core, one BLAS thread each"},
+                                    "host_cores": os.cpu_count()}
         print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

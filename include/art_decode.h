@@ -35,7 +35,7 @@
 extern "C" {
 #endif
 
-#define ART_VERSION 110          /* 0.1.1: art_desc_t.q_len */
+#define ART_VERSION 120          /* 0.2.0: art_desc_t.num_pages, ART_SPLIT_PERSISTENT, art_query_clusters, art_hbm_read_probe */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
 #define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent clusters, cluster size chosen by the library (BF16 only) */
 #define ART_SPLIT_PERSISTENT(cl) (-1 - (cl))   /* art_desc_t.split: persistent clusters of cl = 1..16 CTAs (BF16 only) */
@@ -92,6 +92,8 @@ typedef struct art_desc {
                                   criterion is the AND over all m * G (token, head) rows (reading R15).
                                   m > 1 needs m * G <= 8 and a cluster schedule (split >= 0); q and out are then
                                   [B, m, Hq, d]. */
+  int32_t num_pages;           /* pages in k_cache / v_cache; 0 = not given.  Only read by debug builds of the library
+                                  (-DART_DEBUG), which check every block_table entry a call can reach against it */
   const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
   int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
                                   (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */
@@ -192,6 +194,12 @@ int art_query_split(const art_desc_t* desc, int art_on);
 /* Number of persistent clusters the library would launch for this problem (BF16 only; needs a CUDA device);
  * art_on: 0 = detector off, 1 = probe of 32 coordinates, 2 = full-output detector.  <0 = error code. */
 int art_query_clusters(const art_desc_t* desc, int art_on);
+
+/* Measurement aid: streams the first floor(bytes / 32768) * 32768 bytes of the DEVICE buffer `buf`
+ * (16-byte aligned) through shared memory with the access pattern of the attention kernels (32 KiB TMA bulk copies, a
+ * 3-stage ring, two CTAs per SM) and no compute: the time of this call is the read-only HBM ceiling of the box the
+ * attention kernels are compared with (bench.py: roofline.read_only_ceiling_gbs).  Enqueues on cuda_stream. */
+int art_hbm_read_probe(const void* buf, size_t bytes, void* cuda_stream);
 
 /* Human-readable text for a status code (static storage). */
 const char* art_status_string(int status);

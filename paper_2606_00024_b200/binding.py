@@ -34,7 +34,7 @@ class ArtDesc(C.Structure):
         ("head_dim", C.c_int32), ("block_tokens", C.c_int32), ("dtype", C.c_int32),
         ("kv_layout", C.c_int32), ("policy", C.c_int32), ("max_blocks_per_seq", C.c_int32),
         ("sink_tokens", C.c_int32), ("window_tokens", C.c_int32), ("max_eligible", C.c_int32),
-        ("sm_scale", C.c_float), ("split", C.c_int32), ("q_len", C.c_int32),
+        ("sm_scale", C.c_float), ("split", C.c_int32), ("q_len", C.c_int32), ("num_pages", C.c_int32),
         ("eligible_counts", C.c_void_p), ("blocks_loaded", C.c_void_p),
     ]
 
@@ -51,7 +51,8 @@ class ArtError(RuntimeError):
 
 
 def lib_path() -> str:
-    return os.path.join(_HERE, _LIB_NAME)
+    """The in-tree library; ART_LIB_PATH selects another build of it (the -DART_DEBUG one of tests/test_gpu_debug_build.py)."""
+    return os.environ.get("ART_LIB_PATH") or os.path.join(_HERE, _LIB_NAME)
 
 
 _lib = None
@@ -85,6 +86,8 @@ def load_library():
     lib.art_query_split.argtypes = [C.POINTER(ArtDesc), C.c_int]
     lib.art_query_clusters.restype = C.c_int
     lib.art_query_clusters.argtypes = [C.POINTER(ArtDesc), C.c_int]
+    lib.art_hbm_read_probe.restype = C.c_int
+    lib.art_hbm_read_probe.argtypes = [vp, C.c_size_t, vp]
     lib.art_status_string.restype = C.c_char_p
     lib.art_status_string.argtypes = [C.c_int]
     lib.art_version.restype = C.c_int
@@ -179,6 +182,13 @@ def art_decode_attention_host(desc, q_host, k_cache, v_cache, block_table_host, 
         raise ArtError(rc, "art_decode_attention_host")
 
 
+def art_hbm_read_probe(buf, stream=None) -> None:
+    """Read-only streaming pass over a CUDA tensor (measurement aid, include/art_decode.h)."""
+    rc = load_library().art_hbm_read_probe(_ptr(buf), buf.numel() * buf.element_size(), _stream_ptr(stream))
+    if rc != 0:
+        raise ArtError(rc, "art_hbm_read_probe")
+
+
 def art_topk_blocks(desc, q, k_cache, block_table, seq_lens, top_k, block_scores, eligible_blocks, eligible_counts,
                     stream=None) -> None:
     """Importance-first block list of the scored base policy, built on the device (include/art_decode.h)."""
@@ -202,6 +212,7 @@ def make_desc(w, *, split: int = 0, blocks_loaded=None, eligible_counts=None, sm
         sink_tokens=w.sink_tokens, window_tokens=w.window_tokens,
         max_eligible=0 if w.eligible_blocks is None else int(w.eligible_blocks.shape[2]),
         sm_scale=sm_scale, split=split, q_len=int(w.q.shape[1]) if w.q.dim() == 4 else 0,
+        num_pages=int(w.k_cache.shape[0]),
         eligible_counts=None if ec is None else ec.data_ptr(),
         blocks_loaded=None if blocks_loaded is None else blocks_loaded.data_ptr())
 

@@ -16,6 +16,9 @@
 #include "art_host_util.cuh"
 #include "art_launch.h"
 #include "art_policy.cuh"
+#ifdef ART_DEBUG
+#include "art_debug.cuh"
+#endif
 
 namespace art {
 
@@ -271,8 +274,8 @@ static int choose_pc(int G, int want, int groups, const PcPlan& pl, int* CL_out,
 // steps a CTA of a persistent cluster claims per atomic on its cluster's board
 static int pc_claim() { return 4; }
 
-#ifdef ART_WATCHDOG
-// debugging build: a pinned, device-mapped word that a wait which never ends writes before it traps; it survives
+#if defined(ART_WATCHDOG) || defined(ART_DEBUG)
+// debugging builds: a pinned, device-mapped word that a wait which never ends writes before it traps; it survives
 // the death of the context, so the test harness can print where the kernel was stuck (art_debug_watchdog())
 static unsigned long long* g_watchdog_host = nullptr;
 static unsigned long long* watchdog_word() {
@@ -350,6 +353,10 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const float scale = d->sm_scale > 0.f ? d->sm_scale : 1.0f / sqrtf(static_cast<float>(d->head_dim));
   p.scale_log2 = scale * 1.4426950408889634f;
   if (th) { p.tau = th->tau; p.phi = th->phi; p.patience = th->patience; }
+#ifdef ART_DEBUG
+  debug::art_validate_inputs_kernel<<<groups, 128, 0, stream>>>(p, d->num_pages, watchdog_word() ? watchdog_word() + 4 : nullptr);
+  if (cudaGetLastError() != cudaSuccess) return ART_ERR_CUDA;
+#endif
 
   cudaError_t e;
   if (persistent) {
@@ -676,6 +683,15 @@ int art_version(void) { return ART_VERSION; }
 
 #ifdef ART_WATCHDOG
 unsigned long long art_debug_watchdog(void) { return art::g_watchdog_host ? art::g_watchdog_host[0] : 0ull; }
+#endif
+#ifdef ART_DEBUG
+// (code << 48 | b << 32 | g << 24 | index) of the first violation art_validate_inputs_kernel found, 0 if none; *value gets
+// the offending value.  The word lives in pinned host memory: it can be read after the trap has killed the context.
+unsigned long long art_debug_last_violation(unsigned long long* value) {
+  if (!art::g_watchdog_host) return 0ull;
+  if (value) *value = art::g_watchdog_host[6];
+  return art::g_watchdog_host[5];
+}
 #endif
 
 }  // extern "C"

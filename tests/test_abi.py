@@ -30,7 +30,7 @@ def test_every_declared_symbol_is_exported(art):
             "art_workspace_bytes", "art_query_split", "art_query_clusters", "art_status_string", "art_version"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
-    assert art.art_version() == 110
+    assert art.art_version() == 120
     assert "NULL" in art.art_status_string(-1) and art.art_status_string(0) == "ok"
 
 

@@ -183,6 +183,24 @@ def test_golden_harmonic_trace():
         np.testing.assert_allclose(r.d_direction_all[t - 1], float(dd), atol=1e-12)
 
 
+def test_golden_two_direction_trace():
+    """tests/golden/two_direction_trace.txt: a closed form whose d_direction is neither 0 nor 1 (block 1 = e_a, block 2 =
+    e_b, then e_a again; q = 0): d_direction^(2) = 1 - 1/sqrt(2), d_scale^(t) = sqrt(2) / (t (t - 1)).  Pins Eq. 2's
+    cosine with numbers derived by hand, for two heads and two different coordinate pairs."""
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "two_direction_trace.txt")) if not l.startswith("#")]
+    T, d = len(rows), 64
+    idx = ao.probe_indices(d)
+    for a, b in ((int(idx[0]), int(idx[5])), (int(idx[31]), int(idx[2]))):
+        q = np.zeros((2, d)); K = np.random.default_rng(1).standard_normal((T, N, d))
+        V = np.zeros((T, N, d)); V[:, :, a] = 1.0; V[1, :, a] = 0.0; V[1, :, b] = 1.0
+        r = ao.art_group(q, K, V, np.ones((T, N), bool), 0.0, 0.0, 5, trace=True)
+        assert abs(r.d_direction_all[1, 0] - (1.0 - 1.0 / np.sqrt(2.0))) < 1e-14
+        for t, ds, dd in rows:
+            t = int(t)
+            np.testing.assert_allclose(r.d_scale_all[t - 1], float(ds), rtol=1e-12)
+            np.testing.assert_allclose(r.d_direction_all[t - 1], float(dd), rtol=1e-10, atol=1e-14)
+
+
 @pytest.mark.parametrize("p", [1, 2, 5, 9])
 def test_constant_values_stop_at_p_plus_one(p):
     """Closed form (i): all V rows equal v (v[idx] != 0) => o^(t) = v for all t, so
