@@ -37,21 +37,22 @@ extern "C" {
 
 #define ART_VERSION 120          /* 0.2.0: art_desc_t.num_pages, ART_SPLIT_PERSISTENT, art_query_clusters, art_hbm_read_probe */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
-#define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent clusters, cluster size chosen by the library (BF16 only) */
-#define ART_SPLIT_PERSISTENT(cl) (-1 - (cl))   /* art_desc_t.split: persistent clusters of cl = 1..16 CTAs (BF16 only) */
+#define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent clusters, cluster size chosen by the library (BF16, detector
+                                    off; a call with the detector on runs the library's static clusters instead) */
+#define ART_SPLIT_PERSISTENT(cl) (-1 - (cl))   /* same with clusters of cl = 1..16 CTAs */
 #define ART_PATIENCE_INF 2147483647 /* "p = infinity": detector runs, never fires (App. E) */
 
 /* status codes: 0 = OK, negative = error.  No exceptions, no abort. */
 enum {
   ART_OK = 0,
   ART_ERR_NULL = -1,      /* a required pointer is NULL */
-  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G = Hq / Hkv > 8, q_len * G > 8, q_len > 1 with ART_SPLIT_DYNAMIC,
-                             unsupported head_dim, block_tokens != 64, negative sizes, policy/list mismatch,
-                             bad thresholds */
+  ART_ERR_SHAPE = -2,     /* Hq % Hkv != 0, G = Hq / Hkv > 8, q_len * G > 8, unsupported head_dim, block_tokens != 64,
+                             negative sizes, split outside ART_SPLIT_PERSISTENT(16)..16, BF16 with max_blocks_per_seq
+                             or max_eligible >= 2^24, policy/list mismatch, bad thresholds */
   ART_ERR_DTYPE = -3,     /* dtype / head_dim combination not built (built: F32 d=64, BF16 d=128) */
   ART_ERR_ALIGN = -4,     /* q / k_cache / v_cache not 16-byte aligned */
-  ART_ERR_WORKSPACE = -5, /* workspace NULL, misaligned or too small where one is needed (the *_host entry point,
-                             split == ART_SPLIT_DYNAMIC) */
+  ART_ERR_WORKSPACE = -5, /* workspace NULL, misaligned or too small where one is needed (the *_host entry point;
+                             split < 0 on a detector-off call) */
   ART_ERR_ARCH = -6,      /* current device is not compute capability 10.x */
   ART_ERR_CUDA = -7       /* a CUDA runtime call or the launch failed */
 };
@@ -80,23 +81,32 @@ typedef struct art_desc {
   int32_t window_tokens;       /* SINK_WINDOW */
   int32_t max_eligible;        /* row stride of eligible_blocks (LIST) */
   float sm_scale;              /* logit scale; 0 => 1/sqrt(d) (Eq. 1) */
-  int32_t split;               /* CTAs (thread-block cluster size) cooperating on one group:
-                                  0 = choose automatically, else 1..16 (a power of two for F32), or
-                                  ART_SPLIT_DYNAMIC: no fixed binding, a persistent grid whose CTAs claim steps
-                                  of whichever group has work left (needs `workspace`).  Any value gives the
-                                  same stop_block as the sequential algorithm. */
+  int32_t split;               /* how CTAs are bound to groups.
+                                  1..16 (a power of two for F32): STATIC clusters, one thread-block cluster of that
+                                  many CTAs per group, the steps of the group dealt over its CTAs.
+                                  ART_SPLIT_DYNAMIC / ART_SPLIT_PERSISTENT(cl) (BF16, detector off): PERSISTENT clusters,
+                                  as many as fit the GPU at once; each takes groups from a queue and its CTAs claim
+                                  steps of whichever of the cluster's open groups has work left (needs `workspace`).
+                                  A detector-on call with split < 0 runs static clusters of the library's choice.
+                                  0 = the library decides: static clusters sized so that groups x CTAs fill the GPU,
+                                  except for detector-off BF16 calls with more groups than one-CTA clusters fit at
+                                  once (many short groups), which use persistent clusters when a workspace is given.
+                                  Any value gives the same stop_block as the sequential algorithm. */
   int32_t q_len;               /* m: query tokens per sequence (speculative decode, the tail of a chunked
                                   prefill); 0 or 1 = plain decode.  The m tokens are the LAST m positions of the
                                   sequence (their K/V are in the cache and counted in seq_lens); query token i attends
                                   to the eligible tokens j <= L - m + i; the group walks its blocks once and the
                                   criterion is the AND over all m * G (token, head) rows (reading R15).
-                                  m > 1 needs m * G <= 8 and a cluster schedule (split >= 0); q and out are then
-                                  [B, m, Hq, d]. */
+                                  m > 1 needs m * G <= 8; q and out are then [B, m, Hq, d]. */
   int32_t num_pages;           /* pages in k_cache / v_cache; 0 = not given.  Only read by debug builds of the library
                                   (-DART_DEBUG), which check every block_table entry a call can reach against it */
   const int32_t* eligible_counts; /* DEVICE [B*Hkv] number of list entries per group (LIST only) */
   int32_t* blocks_loaded;      /* optional DEVICE [B*Hkv] out: KV blocks whose loads were issued
-                                  (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB */
+                                  (processed + prefetched-then-discarded): "bytes actually read" / 32 KiB.
+                                  BF16 with the detector on: blocks_loaded - stop_block <= C (stages + 3) + 4 for a
+                                  group that stops early (C = art_query_split, stages = ring depth, 3 with the default
+                                  probe: at most 28 blocks with clusters of 4), 0 for a group that runs to T
+                                  (Appendix A.7) */
 } art_desc_t;
 
 /* Termination thresholds (tau = 1e-5, phi = 1e-3, p = 5).  HOST memory. */
@@ -121,16 +131,19 @@ typedef struct art_thresholds {
  *   out             DEVICE float32 [B, Hq, d]    o^(t*) (Alg. 1 l.18) ([B, m, Hq, d] when q_len = m > 1)
  *   stop_block      DEVICE int32 [B, Hkv]        t* = number of blocks processed, in [0, T];
  *                                                T if the criterion never fired
- *   workspace       DEVICE scratch, 256-B aligned, >= art_workspace_bytes(desc); only read and written when
- *                   desc->split == ART_SPLIT_DYNAMIC (control blocks, step mailboxes, partial states; the
- *                   call zeroes what it needs), may be NULL otherwise
+ *   workspace       DEVICE scratch, 256-B aligned, >= art_workspace_bytes(desc); only the persistent-cluster kernel
+ *                   uses it (partial online-softmax states, [group][CTA of the cluster][G][d + 2] floats, written
+ *                   before they are read: nothing needs zeroing).  May be NULL: split == 0 then stays on static
+ *                   clusters, split < 0 on a detector-off call returns ART_ERR_WORKSPACE
  *
  * seq_lens[b] == 0 or an empty list gives a zero output row and stop_block 0.
  * Reproducibility: stop_block is bit-deterministic for every schedule.  `out` is bit-reproducible when steps are
- * dealt statically (clusters of 1 or > 4, ART-off); when the CTAs of a cluster claim steps at run time (ART-on with
- * clusters of 2-4, ART_SPLIT_DYNAMIC) the order in which partial states are merged depends on the run and `out`
- * agrees to fp32 rounding (<= 1e-5 relative) between runs.
- * Device-side contents (page ids in range, list entries valid) are not validated.
+ * dealt statically (static clusters of 1 or > 4 CTAs, static clusters with the detector off); when CTAs claim steps at
+ * run time (detector on with static clusters of 2-4, persistent clusters) which CTA folds which step depends on the
+ * run and `out` agrees to fp32 rounding (<= 1e-5 relative) between runs.
+ * Device-side contents (page ids in range, list entries valid and distinct, seq_lens within the table) are not
+ * validated by the release build; a library built with -DART_DEBUG runs a checking kernel before every launch that
+ * records the first violation and traps (tests/test_gpu_debug_build.py).
  */
 int art_decode_attention(const art_desc_t* desc, const void* q, const void* k_cache,
                          const void* v_cache, const int32_t* block_table,
@@ -184,15 +197,17 @@ int art_topk_blocks(const art_desc_t* desc, const void* q, const void* k_cache, 
                     int32_t* eligible_counts, void* cuda_stream);
 
 /* DEVICE scratch bytes that cover every entry point for this problem: the staging area of
- * art_decode_attention_host plus the control blocks, mailboxes and partial states of the dynamically
- * scheduled kernel (split == ART_SPLIT_DYNAMIC).  0 on a bad desc.  Needs no CUDA device. */
+ * art_decode_attention_host plus the partial states of the persistent-cluster kernel (BF16: groups x 16 x G x 130
+ * floats).  0 on a bad desc.  Needs no CUDA device. */
 size_t art_workspace_bytes(const art_desc_t* desc);
 
-/* Cluster size the library would pick for desc->split == 0 (needs a CUDA device); <0 = error code. */
+/* CTAs per cluster the library would launch for this descriptor (desc->split as given; needs a CUDA device):
+ * art_on: 0 = detector off, 1 = probe of 32 coordinates, 2 = full-output detector (probe_dim = 0 or d).
+ * <0 = error code. */
 int art_query_split(const art_desc_t* desc, int art_on);
 
-/* Number of persistent clusters the library would launch for this problem (BF16 only; needs a CUDA device);
- * art_on: 0 = detector off, 1 = probe of 32 coordinates, 2 = full-output detector.  <0 = error code. */
+/* Number of persistent clusters the library would launch for this problem when given a workspace, 0 if the call
+ * runs static clusters (one per group); art_on as above; needs a CUDA device.  <0 = error code. */
 int art_query_clusters(const art_desc_t* desc, int art_on);
 
 /* Measurement aid: streams the first floor(bytes / 32768) * 32768 bytes of the DEVICE buffer `buf`
