@@ -35,11 +35,13 @@
 extern "C" {
 #endif
 
-#define ART_VERSION 120          /* 0.2.0: art_desc_t.num_pages, ART_SPLIT_PERSISTENT, art_query_clusters, art_hbm_read_probe */
+#define ART_VERSION 121          /* 0.2.1: art_decode_attention_off_static (no caller workspace); 0.2.0: art_desc_t.num_pages,
+                                    ART_SPLIT_PERSISTENT, art_query_clusters, art_hbm_read_probe */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
 #define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent clusters, cluster size chosen by the library (BF16, detector
                                     off; a call with the detector on runs the library's static clusters instead) */
 #define ART_SPLIT_PERSISTENT(cl) (-1 - (cl))   /* same with clusters of cl = 1..16 CTAs */
+#define ART_STATIC_SCRATCH_BYTES (32u << 20) /* size of the library's built-in scratch array (art_decode_attention_off_static) */
 #define ART_PATIENCE_INF 2147483647 /* "p = infinity": detector runs, never fires (App. E) */
 
 /* status codes: 0 = OK, negative = error.  No exceptions, no abort. */
@@ -54,7 +56,9 @@ enum {
   ART_ERR_WORKSPACE = -5, /* workspace NULL, misaligned or too small where one is needed (the *_host entry point;
                              split < 0 on a detector-off call) */
   ART_ERR_ARCH = -6,      /* current device is not compute capability 10.x */
-  ART_ERR_CUDA = -7       /* a CUDA runtime call or the launch failed */
+  ART_ERR_CUDA = -7,      /* a CUDA runtime call or the launch failed */
+  ART_ERR_SCRATCH_LIMIT = -8 /* art_decode_attention_off_static: the problem needs more than ART_STATIC_SCRATCH_BYTES of
+                             scratch; use art_decode_attention_off with a caller-provided workspace */
 };
 
 enum { ART_DTYPE_F32 = 0, ART_DTYPE_BF16 = 1 };          /* element type of q, k_cache, v_cache */
@@ -160,6 +164,32 @@ int art_decode_attention_off(const art_desc_t* desc, const void* q, const void* 
                              const int32_t* eligible_blocks, const int32_t* seq_lens,
                              float* out, int32_t* stop_block,
                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/*
+ * ART-off on persistent clusters WITHOUT a caller workspace, for callers that cannot allocate device memory (code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Same computation, arguments and
+ * results as art_decode_attention_off with split = ART_SPLIT_DYNAMIC (desc->split: 0 or negative; > 0 =
+ * ART_ERR_SHAPE, static clusters need no scratch; BF16 only, else ART_ERR_DTYPE), but the partial online-softmax
+ * states of the persistent-cluster kernel (art_static_scratch_needed(desc) = B x Hkv x 16 x padded rows x 130 floats,
+ * rows = G x q_len padded to 1, 2, 4, 8) live in a file-scope device array of ART_STATIC_SCRATCH_BYTES = 32 MiB inside
+ * the library, which every GPU that loads the library holds until the process exits (504 groups of 8 rows, 1008 groups
+ * of 4).  A problem that needs more returns ART_ERR_SCRATCH_LIMIT before anything is launched.  The call and
+ * everything under it calls no cudaMalloc / cudaFree / allocating library routine; the array's device address is taken
+ * once per device (cudaGetSymbolAddress, with the calling thread's current device).
+ * ALL calls on a device share the one array, which keeps the previous call's contents: the kernel writes every partial
+ * state before it reads it, so nothing has to start at zero, but two calls that overlap on the GPU (different streams,
+ * or graph branches that may run concurrently) RACE on it.  Serialise them, or use art_decode_attention_off with
+ * separate workspaces.
+ */
+int art_decode_attention_off_static(const art_desc_t* desc, const void* q, const void* k_cache,
+                                    const void* v_cache, const int32_t* block_table,
+                                    const int32_t* eligible_blocks, const int32_t* seq_lens,
+                                    float* out, int32_t* stop_block, void* cuda_stream);
+
+/* ART_STATIC_SCRATCH_BYTES of the loaded library / scratch bytes this problem would need (0 on a bad desc).
+ * Neither needs a CUDA device. */
+size_t art_static_scratch_bytes(void);
+size_t art_static_scratch_needed(const art_desc_t* desc);
 
 /*
  * End-to-end variants for a serving loop: the per-step inputs (q, block_table,

@@ -75,6 +75,12 @@ def load_library():
     lib.art_decode_attention_off.restype = C.c_int
     lib.art_decode_attention_off.argtypes = [C.POINTER(ArtDesc), vp, vp, vp, i32p, i32p, i32p,
                                              f32p, i32p, vp, C.c_size_t, vp]
+    lib.art_decode_attention_off_static.restype = C.c_int
+    lib.art_decode_attention_off_static.argtypes = [C.POINTER(ArtDesc), vp, vp, vp, i32p, i32p, i32p, f32p, i32p, vp]
+    lib.art_static_scratch_bytes.restype = C.c_size_t
+    lib.art_static_scratch_bytes.argtypes = []
+    lib.art_static_scratch_needed.restype = C.c_size_t
+    lib.art_static_scratch_needed.argtypes = [C.POINTER(ArtDesc)]
     lib.art_decode_attention_host.restype = C.c_int
     lib.art_decode_attention_host.argtypes = [C.POINTER(ArtDesc), vp, vp, vp, i32p, i32p, i32p,
                                               C.POINTER(ArtThresholds), f32p, i32p, vp, C.c_size_t, vp]
@@ -167,6 +173,25 @@ def art_decode_attention_off(desc, q, k_cache, v_cache, block_table, eligible_bl
         _ptr(seq_lens), _ptr(out), _ptr(stop_block), ws_ptr, ws_bytes, _stream_ptr(stream))
     if rc != 0:
         raise ArtError(rc, "art_decode_attention_off")
+
+
+def art_decode_attention_off_static(desc, q, k_cache, v_cache, block_table, eligible_blocks, seq_lens,
+                                    out, stop_block, stream=None) -> None:
+    """ART-off on persistent clusters with the library's built-in scratch array: no workspace, no allocation
+    (include/art_decode.h).  Calls that overlap on the GPU race on that array."""
+    rc = load_library().art_decode_attention_off_static(
+        C.byref(desc), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_table), _ptr(eligible_blocks),
+        _ptr(seq_lens), _ptr(out), _ptr(stop_block), _stream_ptr(stream))
+    if rc != 0:
+        raise ArtError(rc, "art_decode_attention_off_static")
+
+
+def art_static_scratch_bytes() -> int:
+    return int(load_library().art_static_scratch_bytes())
+
+
+def art_static_scratch_needed(desc: ArtDesc) -> int:
+    return int(load_library().art_static_scratch_needed(C.byref(desc)))
 
 
 def art_decode_attention_host(desc, q_host, k_cache, v_cache, block_table_host, eligible_blocks_host,

@@ -261,7 +261,7 @@ static int choose_split(const art_desc_t* d, int mode, int want, int* C_out) {
 
 // Persistent clusters (detector off): cluster size CL and the number of clusters NC = min(co-resident clusters, groups).
 // The library's own choice is clusters of ONE CTA: measured on configs[3] (1024 groups of ~65 blocks), 355 us against
-// 372 / 363 us with clusters of 2 / 4 and 368 us with static one-CTA clusters (profiles/r02_persistent.md); larger
+// 372 / 363 us with clusters of 2 / 4 and 368 us with static one-CTA clusters (profiles/r02_sweeps.md); larger
 // clusters exist for callers whose groups are few and uneven (the tail of the call is then shared inside a cluster).
 static int choose_pc(int G, int want, int groups, const PcPlan& pl, int* CL_out, int* NC_out) {
   const int CL = want > 0 ? want : 1;
@@ -675,6 +675,7 @@ const char* art_status_string(int status) {
     case ART_ERR_WORKSPACE: return "workspace missing, misaligned or too small";
     case ART_ERR_ARCH: return "device is not compute capability 10.x (sm_100)";
     case ART_ERR_CUDA: return "CUDA runtime or launch error";
+    case ART_ERR_SCRATCH_LIMIT: return "problem needs more scratch than the library's built-in array (ART_STATIC_SCRATCH_BYTES)";
     default: return "unknown status";
   }
 }

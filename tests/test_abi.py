@@ -27,10 +27,12 @@ def test_every_declared_symbol_is_exported(art):
     lib = art.load_library()
     syms = declared_symbols()
     assert {"art_decode_attention", "art_decode_attention_off", "art_decode_attention_host", "art_topk_blocks",
-            "art_workspace_bytes", "art_query_split", "art_query_clusters", "art_status_string", "art_version"} <= set(syms)
+            "art_workspace_bytes", "art_query_split", "art_query_clusters", "art_status_string", "art_version",
+            "art_hbm_read_probe", "art_decode_attention_off_static", "art_static_scratch_bytes",
+            "art_static_scratch_needed"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
-    assert art.art_version() == 120
+    assert art.art_version() == 121
     assert "NULL" in art.art_status_string(-1) and art.art_status_string(0) == "ok"
 
 
@@ -97,3 +99,23 @@ def test_no_gpu_means_loud_failure_not_fallback(art):
     rc = _call_off(art, good_desc(art))
     assert rc in (-6, -7)                                                    # ART_ERR_ARCH / ART_ERR_CUDA
     assert art.art_workspace_bytes(good_desc(art)) > 0
+
+
+def test_static_scratch_sizes_and_limit_need_no_device(art):
+    """art_decode_attention_off_static rejects what does not fit its built-in array before any CUDA call."""
+    import torch
+    from workloads import generators as gen
+    assert art.art_static_scratch_bytes() == 32 << 20
+    w = gen.config(1, scale=1 / 8, batch=2)
+    d = art.make_desc(w)
+    assert art.art_static_scratch_needed(d) == 2 * 8 * 16 * 4 * 130 * 4
+    big = art.ArtDesc(batch=128, num_q_heads=32, num_kv_heads=8, head_dim=128, block_tokens=64, dtype=art.ART_DTYPE_BF16,
+                      max_blocks_per_seq=8)
+    assert art.art_static_scratch_needed(big) > art.art_static_scratch_bytes()
+    lib = art.load_library()
+    x = torch.zeros(64)                                             # never dereferenced: the call fails on the size
+    rc = lib.art_decode_attention_off_static(C.byref(big), x.data_ptr(), x.data_ptr(), x.data_ptr(), x.data_ptr(), None,
+                                             x.data_ptr(), x.data_ptr(), x.data_ptr(), None)
+    assert rc == -8 and "scratch" in art.art_status_string(rc)
+    bad = art.ArtDesc(batch=1, num_q_heads=4, num_kv_heads=1, head_dim=64, block_tokens=64, dtype=art.ART_DTYPE_F32)
+    assert lib.art_decode_attention_off_static(C.byref(bad), *([x.data_ptr()] * 4), None, *([x.data_ptr()] * 3), None) == -3
