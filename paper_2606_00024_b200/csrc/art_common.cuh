@@ -50,7 +50,7 @@ struct Params {
 };
 
 #ifdef ART_TRACE   // debugging aid (never in the shipped build): timestamped events of the first CTAs
-constexpr int kTraceCtas = 8, kTraceRoles = 3, kTraceEvents = 2048;
+constexpr int kTraceCtas = 8, kTraceRoles = 6, kTraceEvents = 1024;
 __device__ __forceinline__ unsigned long long trace_now() {
   unsigned long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t;
 }
@@ -63,7 +63,7 @@ struct Tracer {      // roles claim one of kTraceCtas trace slots when they firs
     if (region == nullptr) return;
     if (!buf) {
       int slot;
-      if (role == 1) { slot = *share - 1; if (slot < 0) return; }            // fold follows its producer
+      if (role != 0) { slot = *share - 1; if (slot < 0) return; }            // every other role follows its producer
       else {
         if (n < 0) return;
         slot = atomicAdd(reinterpret_cast<int*>(region) + role, 1);

@@ -477,7 +477,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     // ===================================================== A5: P~V_t = V_t^T P^T, rows = d, columns = heads
     if (lane == 0) {
       const uint64_t dV = kDescSw128 | desc_strides(kBoxBytes, 1024);
-      const uint64_t dP = kDescNoSw | desc_strides(LBO_P, 128);
+      const uint64_t dP = kDescNoSw | desc_strides(LBO_P, PBUF);   // rows 0-7 = hi, rows 8-15 = lo (art_decode_tc.cuh)
       int st = 0; uint32_t ph = 0;
       for (int i = 0;; ++i) {
         const int ps = i & (NP - 1);
@@ -489,11 +489,9 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
           const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
           const uint32_t pb = sbase + sm.pb + st * 2 * PBUF;
 #pragma unroll
-          for (int part = 0; part < 2; ++part)
-#pragma unroll
-            for (int ks = 0; ks < 4; ++ks)
-              umma_bf16(tmem_PV + ps * kUmmaN, dV | desc_addr(vt + ks * 2048),
-                        dP | desc_addr(pb + part * PBUF + ks * 2 * LBO_P), kIdescPV, (part | ks) > 0);
+          for (int ks = 0; ks < 4; ++ks)
+            umma_bf16(tmem_PV + ps * kUmmaN, dV | desc_addr(vt + ks * 2048),
+                      dP | desc_addr(pb + ks * 2 * LBO_P), kIdescPV, ks > 0);
         }
         umma_commit(bar(sm.empty0 + st));
         umma_commit(bar(sm.pvfull0 + ps));
@@ -608,9 +606,12 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
     };
     auto fold = [&](int i) {
       tc_fence_after();
-      float pv[G];
+      float pv[G], pvl[G];
       tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN, pv);
+      tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN + 8, pvl);
       tmem_ld_wait();
+#pragma unroll
+      for (int h = 0; h < G; ++h) pv[h] += pvl[h];            // hi + lo halves of p
       const float* sl = slots + (i & (kIterSlots - 1)) * 2 * G;
 #pragma unroll
       for (int h = 0; h < G; ++h) {

@@ -17,7 +17,7 @@
 //                                 warps are stateless), split into bf16 hi + lo (~16 mantissa bits, so the
 //                                 probe of P~V_t is accurate to ~1e-5 and the criterion does not flip) and
 //                                 written to shared memory as the B operand of the P.V MMA
-//   PV-MMA   (warp 3, 1 thr) A5   PV[d, head] = V_t^T . P^T : tcgen05.mma M128 N16 K16 x 4 x (hi, lo)
+//   PV-MMA   (warp 3, 1 thr) A5   PV[d, head] = V_t^T . P^T : tcgen05.mma M128 N16 K16 x 4, N = (hi of 8 heads | lo of 8 heads)
 //   fold     (warps 8-11)  A5/A6  one thread per output coordinate: tcgen05.ld of P~V_t; publishes the step
 //                                 summary (m_blk, block sum, probe components of P~V_t) to the cluster
 //                                 leader's mailbox (st.async + mbarrier complete_tx, no fences) and merges
@@ -479,10 +479,13 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       const uint64_t dQ = kDescNoSw | desc_strides(kQLbo, kQSbo);
       const uint32_t qb = sbase + sm.qb;
       int st = 0; uint32_t ph = 0;
+      TC_TRACE_INIT(trm, 3);
       for (int i = 0; i < n_lim; ++i) {
         const int q = i & (NS - 1);
         if (!wait_item(bar(sm.full0 + st), ph, i)) break;
+        TC_TRACE(trm, 2, i, 0);
         if (i >= NS && !wait_item(bar(sm.sfree0 + q), ((i / NS) - 1) & 1, i)) break;
+        TC_TRACE(trm, 10, i, 0);
         tc_fence_after();
         // M = 128 rows are read starting 32 q token rows BELOW the tile (tokens 0-31 -> TMEM lanes 32q..32q+31,
         // columns +0) and once more 32 rows further up (tokens 32-63 -> the same lanes, columns +16).  The
@@ -506,21 +509,25 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     // ===================================================== A5: P~V_t = V_t^T P^T, rows = d, columns = heads
     if (lane == 0) {
       const uint64_t dV = kDescSw128 | desc_strides(kBoxBytes, 1024);  // V tile as V^T: MN-major, 128-B swizzle
-      const uint64_t dP = kDescNoSw | desc_strides(LBO_P, 128);
+      // P^T (hi) and P^T (lo) are ONE B operand of N = 16 rows: rows 0-7 = hi of heads 0-7, rows 8-15 = lo (the stride
+      // between the two 8-row groups is the distance of the lo buffer), so P~V_t costs 4 MMAs: accumulator columns
+      // 0-7 = V^T hi, 8-15 = V^T lo, added by whoever reads them (an MMA costs what its A operand costs to read)
+      const uint64_t dP = kDescNoSw | desc_strides(LBO_P, PBUF);
       int st = 0; uint32_t ph = 0;
+      TC_TRACE_INIT(trv, 5);
       for (int i = 0; i < n_lim; ++i) {
         const int ps = i & (NP - 1);
         if (!wait_item(bar(sm.pfull0 + st), ph, i)) break;
+        TC_TRACE(trv, 6, i, 0);
         if (i >= NP && !wait_item(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1, i)) break;
+        TC_TRACE(trv, 11, i, 0);
         tc_fence_after();
         const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
         const uint32_t pb = sbase + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF;
 #pragma unroll
-        for (int part = 0; part < 2; ++part)                  // p = hi + lo
-#pragma unroll
-          for (int ks = 0; ks < 4; ++ks)                      // 4 x 16 = tokens of the block
-            umma_bf16(tmem_PV + ps * kUmmaN, dV | desc_addr(vt + ks * 2048),
-                      dP | desc_addr(pb + part * PBUF + ks * 2 * LBO_P), kIdescPV, (part | ks) > 0);
+        for (int ks = 0; ks < 4; ++ks)                        // 4 x 16 = tokens of the block; p = hi + lo side by side
+          umma_bf16(tmem_PV + ps * kUmmaN, dV | desc_addr(vt + ks * 2048),
+                    dP | desc_addr(pb + ks * 2 * LBO_P), kIdescPV, ks > 0);
         umma_commit(bar(sm.empty0 + st));                     // K/V stage and its P buffer are free again
         umma_commit(bar(sm.pvfull0 + ps));
         if (++st == S) { st = 0; ph ^= 1u; }
@@ -533,8 +540,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     const int q = warp - kWarpSoftmax0;                       // TMEM lane quadrant == warp % 4; owns blocks i = q (mod 4)
     const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
     int st = q % S;                                           // ring stage of block i
+    TC_TRACE_INIT(trx, 4);
     for (int i = q; i < n_lim; i += NS) {
       if (!wait_item(bar(sm.sfull0 + q), (i / NS) & 1, i)) break;
+      if (q == 0 && lane == 0) TC_TRACE(trx, 3, i, 0);
       tc_fence_after();
       float s0[G], s1[G];
       tmem_ld<G>(taddr, s0);
@@ -604,6 +613,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       }
       fence_proxy_async();                                    // P^T (and V fixes) visible to the tensor core
       mbar_arrive(bar(sm.pfull0 + st));
+      if (q == 0 && lane == 0) TC_TRACE(trx, 9, i, 0);
       st += NS; while (st >= S) st -= S;
     }
   } else if (warp < kWarpFold0 + 4) {
@@ -618,9 +628,12 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     // merge block i (its P~V_t is relative to its own block maximum) into the running state
     auto fold = [&](int i) {
       tc_fence_after();
-      float pv[G];
+      float pv[G], pvl[G];
       tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN, pv);
+      tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN + 8, pvl);
       tmem_ld_wait();
+#pragma unroll
+      for (int h = 0; h < G; ++h) pv[h] += pvl[h];            // hi + lo halves of p
       const IterSlot& sl = slots[i & (kIterSlots - 1)];
 #pragma unroll
       for (int h = 0; h < G; ++h) {
@@ -659,15 +672,18 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (pub < ntot && pub < n_lim && pub - fld < NP) {
           const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
           const uint32_t par = (pub / NP) & 1;
-          if (!pub_ready) pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
+          if (!pub_ready) { pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par); if (pub_ready && tid == 0) TC_TRACE(trf, 7, pub, 0); }
           if (pub_ready && c < 0) { ++pub; pub_ready = false; continue; }   // fired: an unpublished step lies beyond t*
           const int t = pub_ready ? item_step(item_t[pub % kItemT]) : 0;
           if (pub_ready && c >= t - M) {                      // mailbox slot free: step t - M has been scanned
             const int slot_i = (t - 1) & (M - 1);
             tc_fence_after();
-            float pv[G];
+            float pv[G], pvl[G];
             tmem_ld<G>(tmem_PV + tlane + (pub & (NP - 1)) * kUmmaN, pv);
+            tmem_ld<G>(tmem_PV + tlane + (pub & (NP - 1)) * kUmmaN + 8, pvl);
             tmem_ld_wait();
+#pragma unroll
+            for (int h = 0; h < G; ++h) pv[h] += pvl[h];
             const IterSlot& sl = slots[pub & (kIterSlots - 1)];
             const uint32_t row0 = mapa(sbase + sm.mbox + static_cast<uint32_t>(slot_i) * kSummaryBytes, 0);
             const uint32_t mb = mapa(bar(sm.mbox0 + slot_i), 0);
@@ -729,7 +745,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         mbar_arrive_expect_tx(bar(sm.mbox0 + ((i0 + lane) & (M - 1))), kSummaryBytes);
       __syncwarp();
       const int t_last = fired >= 0 ? t + fired : t + n - 1;
-      if (lane == 0) TC_TRACE(trs, 8, t, n);
+      if (lane == 0) TC_TRACE(trs, 8, (group << 12) | t, n);
       if (lane < C) st_cluster_relaxed_s32(mapa(a_ctrl, lane), fired >= 0 ? -t_last : t_last);
       if (fired >= 0) { t_stop = t_last; break; }
       t += n;
