@@ -300,6 +300,13 @@ static int static_run_ahead(int C, int stages) {
   return C * (stages + 3) + 4;
 }
 
+// static bf16 clusters, detector on: how long a fold warp that can neither publish nor merge sleeps before it looks again
+// (a warp that polls takes issue slots from the softmax, MMA-issue and scan warps of its scheduler).  ART_FOLD_SLEEP overrides.
+static int fold_sleep_ns() {
+  static const int env = [] { const char* e = getenv("ART_FOLD_SLEEP"); return e ? atoi(e) : -1; }();
+  return env >= 0 ? env : 0;
+}
+
 // workspace of the persistent-cluster kernel: one partial state (m, l, acc) per (group, CTA of a cluster)
 static size_t pc_part_bytes(int groups, int G) {
   return static_cast<size_t>(groups) * pc::kMaxCL * static_cast<size_t>(G * (tc::kD + 2)) * 4u;
@@ -393,9 +400,11 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
     // static bf16 clusters: with the detector on, steps are claimed at run time for clusters of 2-4 (measured in round 1)
     p.dyn = (tensor_core && mode != 0 && C >= 2 && C <= 4) ? 1 : 0;
     p.run_ahead = (tensor_core && mode != 0) ? static_run_ahead(C, pl.stages) : 0;
+    p.fold_sleep = fold_sleep_ns();
     if (tensor_core) {
 #ifdef ART_TRACE
       if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
+      { const char* e = getenv("ART_DBG"); p.dbg = e ? atoi(e) : 0; if (p.dbg & 8) p.dyn = 0; if (p.dbg & 16) p.dyn = (mode != 0); }
 #endif
       CUtensorMap tmK, tmV;
       if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))

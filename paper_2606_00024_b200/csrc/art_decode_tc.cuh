@@ -8,15 +8,17 @@
 //
 //   producer (warp 0)      A1/A2  resolves block -> page, issues 4 TMA tensor boxes (K, V: two 64-column
 //                                 halves each, 128-byte swizzle) into the ring of stages
-//   S-MMA    (warp 1, 1 thr) A3   S[token, head] = K_t . Q^T : tcgen05.mma M128 N16 K16, issued twice per
-//                                 k-step so that tokens 0-31 and 32-63 of the block land in the SAME 32
-//                                 TMEM lanes (columns +0 / +16) of the softmax warp that owns the block
-//   softmax  (warps 4-7)   A4     warp q owns blocks i = q (mod 4): one warp sees all 64 tokens (two per
-//                                 thread), so the block maximum is one redux per head and no warp ever
-//                                 waits for another.  p = 2^(s - m_blk) relative to the BLOCK maximum (the
-//                                 warps are stateless), split into bf16 hi + lo (~16 mantissa bits, so the
-//                                 probe of P~V_t is accurate to ~1e-5 and the criterion does not flip) and
-//                                 written to shared memory as the B operand of the P.V MMA
+//   S-MMA    (warp 1, 1 thr) A3   S[token, head] = K_t . Q^T : tcgen05.mma M128 N16 K16, ONE per k-step: the 64
+//                                 tokens are M rows 0-63 (even blocks; TMEM lanes 0-63) or rows 64-127 (odd
+//                                 blocks: the operand starts 64 rows below the tile; lanes 64-127).  What an MMA
+//                                 costs here is reading its A operand (128 rows x 32 B) from shared memory, so
+//                                 the K tile is read twice per block, not four times as in round 1
+//   softmax  (warps 4-7)   A4     a PAIR of warps owns a block (warps 4, 5: even blocks; 6, 7: odd blocks), one
+//                                 token per thread; the two halves exchange their maxima through shared memory
+//                                 and one 64-thread named barrier.  p = 2^(s - m_blk) relative to the BLOCK
+//                                 maximum (the warps are stateless), split into bf16 hi + lo (~16 mantissa
+//                                 bits, so the probe of P~V_t is accurate to ~1e-5 and the criterion does not
+//                                 flip) and written to shared memory as the B operand of the P.V MMA
 //   PV-MMA   (warp 3, 1 thr) A5   PV[d, head] = V_t^T . P^T : tcgen05.mma M128 N16 K16 x 4, N = (hi of 8 heads | lo of 8 heads)
 //   fold     (warps 8-11)  A5/A6  one thread per output coordinate: tcgen05.ld of P~V_t; publishes the step
 //                                 summary (m_blk, block sum, probe components of P~V_t) to the cluster
@@ -41,7 +43,13 @@ namespace tc {
 #ifdef ART_TRACE
 #define TC_TRACE_INIT(tr, role) Tracer tr; tr.init(p.trace, 0, role, reinterpret_cast<volatile int*>(smem + sm.misc + 20))
 #define TC_TRACE(tr, code, a, b) tr.ev(code, a, b)
+#define TC_DBG(bit) ((p.dbg & (bit)) != 0)
+#define TC_CLK(v) const long long v = clock64()
+#define TC_ACC(k, a, b) do { clk_acc[k] += (b) - (a); ++clk_cnt[k]; } while (0)
 #else
+#define TC_DBG(bit) false
+#define TC_CLK(v)
+#define TC_ACC(k, a, b)
 #define TC_TRACE_INIT(tr, role)
 #define TC_TRACE(tr, code, a, b)
 #endif
@@ -55,13 +63,16 @@ constexpr int kUmmaN = 16;                   // MMA N: the group's heads padded 
 constexpr int kSSlots = 4;                   // S accumulators: one per softmax warp, 2 x 16 TMEM columns
 constexpr int kSCols = 2 * kUmmaN;
 constexpr int kPVSlots = 8;                  // unfolded P~V_t results (16 TMEM columns each)
-constexpr int kTmemCols = 256;               // 4 x 32 + 8 x 16; two CTAs share the SM's 512 columns
+constexpr int kSCols1 = kUmmaN;              // static-cluster kernel: an S accumulator is 16 columns (64 tokens on the lanes)
+constexpr int kTmemCols = 256;               // S + 8 x 16 (allocations are powers of two); two CTAs share the SM's 512 columns
 constexpr int kIterSlots = 16;               // softmax -> fold hand-over ring; >= kPVSlots + max stages
 constexpr int kMaxStages = 6;
 // P^T (hi, lo) buffers: one per ring stage, except for G = 8 with the detector on, where shared memory only has room for two (block i
 // then uses buffer i & 1, free again once P~V_(i-2) is complete)
 // ring of the step numbers of the items in flight (>= stages + kPVSlots entries; 12 where every byte counts)
 __host__ __device__ constexpr int item_ring(int G, bool art32) { return (G == 8 && art32) ? 12 : 16; }
+// softmax -> fold hand-over ring of the static-cluster kernel: per block [m_blk | block sum of tokens 0-31 | of tokens 32-63] x G
+__host__ __device__ constexpr int iter_ring(int G, bool art32) { return (G == 8 && art32) ? 12 : kIterSlots; }
 __host__ __device__ constexpr int p_bufs(int G, int stages, bool art32) { return (G == 8 && art32) ? 2 : stages; }
 constexpr int kBoxBytes = 8192;              // one TMA box: 64 rows x 128 bytes
 constexpr int kFront = 12288;                // mapped bytes the S MMA may read below a K tile (3 x 32 rows)
@@ -73,15 +84,10 @@ static_assert(kIterSlots >= kPVSlots + kMaxStages, "IterSlot ring too short");
 // P^T as B operand: [8 token-chunks of 8][rows][16 B]; chunk stride 16 G + 16 B puts the 4 chunks a warp
 // writes at once into distinct banks; rows >= G alias later chunks (unread accumulator columns).
 __host__ __device__ constexpr int p_lbo(int G) { return 16 * G + 16; }
-__host__ __device__ constexpr int p_buf_bytes(int G) { return 7 * p_lbo(G) + 256; }
-
-struct IterSlot {            // what softmax hands to fold for one block
-  float mref[8];             // m_blk: block maximum of the scaled logits (log2 domain) = reference of p
-  float lsum[8];             // sum of the block's (rounded) p
-};
+__host__ __device__ constexpr int p_buf_bytes(int G) { return 7 * p_lbo(G) + 128; }
 
 struct SmemMap {
-  uint32_t qb, pb, slots, items, sinfo, mbox, bars, misc, ring, total;
+  uint32_t qb, pb, slots, xch, items, sinfo, mbox, bars, misc, ring, total;
   uint32_t full0, empty0, pfull0, sfull0, sfree0, pvfull0, pvfree0, done0, mbox0, nbars;
 };
 
@@ -92,7 +98,8 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   uint32_t off = 0;
   m.qb = off; off += kQBytes;
   m.pb = off; off += static_cast<uint32_t>(p_bufs(G, stages, art && PW == 32)) * 2u * p_buf_bytes(G);
-  m.slots = off; off += kIterSlots * static_cast<uint32_t>(sizeof(IterSlot));
+  m.slots = off; off += static_cast<uint32_t>(iter_ring(G, art && PW == 32)) * 3u * G * 4u;
+  m.xch = off; off += 8u * G * 4u;        // block maxima of the two token halves: [pair][parity][half][G]
   m.items = off; off += static_cast<uint32_t>(item_ring(G, art && PW == 32)) * 4u;
   m.sinfo = off; off += static_cast<uint32_t>(stages) * 8u;
   off = (off + 15u) & ~15u;                // mailbox rows are written with 16-byte st.async
@@ -114,7 +121,7 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   m.total = off;
   return m;
 }
-constexpr uint32_t kCtrl = 0, kLoaded = 4, kTmemPtr = 8, kNext = 12, kNTotal = 16;
+constexpr uint32_t kCtrl = 0, kNTotal = 4, kLoaded = 8, kTmemPtr = 12, kNext = 16;   // (ctrl, n_total) are read as one 8-byte word
 
 // An entry of the item ring: the step number in the low 24 bits and, for multi-token queries (R15), the causal
 // code of the step's block above them: e = L - 64 * blk (tokens of the sequence from the start of this block on)
@@ -207,6 +214,10 @@ __device__ __forceinline__ void st_cluster_relaxed_s32(uint32_t cluster_addr, in
 __device__ __forceinline__ int ld_ctrl_relaxed(uint32_t addr) {
   int v; asm volatile("ld.relaxed.cluster.shared::cta.s32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory"); return v;
 }
+// the progress word and the number of items the producer will issue, in one load (x = ctrl, y = n_total)
+__device__ __forceinline__ int2 ld_ctrl_ntotal(uint32_t addr) {
+  int2 v; asm volatile("ld.relaxed.cluster.shared::cta.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr) : "memory"); return v;
+}
 
 // Sum G per-lane values over the 32 lanes with a transposing butterfly (G-1 + 5-log2(G) ... shuffles instead
 // of 5 G): afterwards v[0] of lane l holds the total of value head_of_lane32<G>(l).
@@ -260,7 +271,9 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   const uint32_t bars = sbase + sm.bars;
   auto bar = [&](uint32_t idx) { return bars + idx * 8u; };
   const uint32_t a_ctrl = sbase + sm.misc + kCtrl, a_loaded = sbase + sm.misc + kLoaded, a_tmem = sbase + sm.misc + kTmemPtr;
-  IterSlot* slots = reinterpret_cast<IterSlot*>(smem + sm.slots);
+  constexpr int kIterN = iter_ring(G, MODE == 1);
+  float* slots = reinterpret_cast<float*>(smem + sm.slots);   // block i: slots + (i % kIterN) * 3 G = [m_blk | sum lo half | sum hi half][G]
+  float* xch = reinterpret_cast<float*>(smem + sm.xch);
   unsigned long long* sinfo = reinterpret_cast<unsigned long long*>(smem + sm.sinfo);   // [S] token masks
   float* mbox = reinterpret_cast<float*>(smem + sm.mbox);
 
@@ -285,8 +298,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
 #endif
   // ---- one-time setup: barriers, tensor memory, Q^T
   if (tid == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 32); }
-    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 1); }
+    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 64); }
+    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 2); }
     for (int s = 0; s < NP; ++s) { mbar_init(bar(sm.pvfull0 + s), 1); mbar_init(bar(sm.pvfree0 + s), 4); }
     mbar_init(bar(sm.done0), 1); mbar_init(bar(sm.done0 + 1), 1);
     if (ART) {
@@ -317,7 +330,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   cluster_sync_all();           // barriers of every CTA of the cluster are live before any remote store
   tc_fence_after();
   const uint32_t tmem_base = static_cast<uint32_t>(ld_volatile_s32(a_tmem));
-  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kSCols;
+  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kSCols1;
 
   // "fired and step t lies beyond t*": every wait that could otherwise never end checks this
   auto beyond_stop = [&](int t) -> bool {
@@ -487,17 +500,15 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         if (i >= NS && !wait_item(bar(sm.sfree0 + q), ((i / NS) - 1) & 1, i)) break;
         TC_TRACE(trm, 10, i, 0);
         tc_fence_after();
-        // M = 128 rows are read starting 32 q token rows BELOW the tile (tokens 0-31 -> TMEM lanes 32q..32q+31,
-        // columns +0) and once more 32 rows further up (tokens 32-63 -> the same lanes, columns +16).  The
-        // other 96 rows are whatever lies next to the tile and only feed lanes nobody reads.
-        const uint32_t kt = sbase + sm.ring + st * kStageBytes - q * 4096;
-        const uint32_t dcol = tmem_S + q * kSCols;
+        // M = 128 rows are read starting at the tile (even blocks: tokens 0-63 -> TMEM lanes 0-63) or 64 token rows
+        // BELOW it (odd blocks: tokens 0-63 -> lanes 64-127).  The other 64 rows are whatever lies next to the tile
+        // and only feed lanes nobody reads.
+        const uint32_t kt = sbase + sm.ring + st * kStageBytes - (i & 1) * kBoxBytes;
+        const uint32_t dcol = tmem_S + q * kSCols1;
 #pragma unroll
         for (int ks = 0; ks < 8; ++ks) {                      // 8 x 16 = head_dim
           const uint32_t ka = kt + (ks >> 2) * kBoxBytes + (ks & 3) * 32;
-          const uint64_t bq = dQ | desc_addr(qb + ks * 2 * kQLbo);
-          umma_bf16(dcol, dK | desc_addr(ka), bq, kIdescS, ks > 0);
-          umma_bf16(dcol + kUmmaN, dK | desc_addr(ka + 4096), bq, kIdescS, ks > 0);
+          umma_bf16(dcol, dK | desc_addr(ka), dQ | desc_addr(qb + ks * 2 * kQLbo), kIdescS, ks > 0);
         }
         umma_commit(bar(sm.sfull0 + q));
         if (++st == S) { st = 0; ph ^= 1u; }
@@ -536,85 +547,81 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       mbar_wait(bar(sm.done0 + 1), 0);
     }
   } else if (warp >= kWarpSoftmax0 && warp < kWarpSoftmax0 + 4) {
-    // ===================================================== A4: block-local softmax, two tokens per thread
-    const int q = warp - kWarpSoftmax0;                       // TMEM lane quadrant == warp % 4; owns blocks i = q (mod 4)
-    const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
-    int st = q % S;                                           // ring stage of block i
+    // ===================================================== A4: block-local softmax, one token per thread, two warps per block
+    const int q = warp - kWarpSoftmax0;                       // TMEM lane quadrant == warp % 4
+    const int pair = q >> 1, half = q & 1;                    // the pair owns blocks i = pair (mod 2); this warp tokens 32 half + lane
+    const int tok = half * 32 + lane;
+    const uint32_t tq = static_cast<uint32_t>(q * 32) << 16;
+    int st = pair % S;                                        // ring stage of block i
     TC_TRACE_INIT(trx, 4);
-    for (int i = q; i < n_lim; i += NS) {
-      if (!wait_item(bar(sm.sfull0 + q), (i / NS) & 1, i)) break;
+    for (int i = pair; i < n_lim; i += 2) {
+      const int sslot = i & (NS - 1);
+      if (!wait_item(bar(sm.sfull0 + sslot), (i / NS) & 1, i)) break;
       if (q == 0 && lane == 0) TC_TRACE(trx, 3, i, 0);
       tc_fence_after();
-      float s0[G], s1[G];
-      tmem_ld<G>(taddr, s0);
-      tmem_ld<G>(taddr + kUmmaN, s1);
+      float sv[G];
+      tmem_ld<G>(tmem_S + sslot * kSCols1 + tq, sv);
       tmem_ld_wait();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+      if (lane == 0) mbar_arrive(bar(sm.sfree0 + sslot));
       // P^T buffer i & 1 is read by the P.V MMA of block i - 2: wait until that one is complete
       if (kTwoPBufs && i >= 2 && !wait_item(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1, i)) break;
       const unsigned long long vmask = sinfo[st];             // written before the loads the S MMA waited for
-      const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
+      const bool v0 = (vmask >> tok) & 1ull;
       float mb[G];
       int ec = 0;
       if constexpr (MT) ec = item_t[i % kItemT] >> kItemShift;
-      if (MT && ec != 0) {                                    // R15: the most recent tokens are cut row by row
 #pragma unroll
-        for (int h = 0; h < G; ++h) {
-          const int lim = ec - static_cast<int>((p.cuts >> (4 * h)) & 15u);
-          s0[h] = (v0 && lane < lim) ? s0[h] * p.scale_log2 : kNegInf;
-          s1[h] = (v1 && lane + 32 < lim) ? s1[h] * p.scale_log2 : kNegInf;
-          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
-        }
-      } else {
-#pragma unroll
-        for (int h = 0; h < G; ++h) {
-          s0[h] = v0 ? s0[h] * p.scale_log2 : kNegInf;        // masked tokens: weight 0 (R8); their K may be NaN
-          s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
-          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
-        }
+      for (int h = 0; h < G; ++h) {
+        bool vis = v0;                                        // masked tokens: weight 0 (R8); their K may be NaN
+        if (MT && ec != 0) vis = vis && tok < ec - static_cast<int>((p.cuts >> (4 * h)) & 15u);   // R15: causal cut row by row
+        sv[h] = vis ? sv[h] * p.scale_log2 : kNegInf;
+        mb[h] = warp_max_f32(sv[h]);
       }
-      uint8_t* pb0 = smem + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;   // token `lane`, row 0, hi
+      {
+        // block maximum = max over the two halves: through shared memory and the pair's named barrier.  The area is
+        // double-buffered by block parity: a warp can be at most one block ahead of its partner at the barrier.
+        float* xw = xch + (((pair * 2 + ((i >> 1) & 1)) * 2) + half) * G;
+        const float* xr = xch + (((pair * 2 + ((i >> 1) & 1)) * 2) + (half ^ 1)) * G;
+        float mine = mb[0];
+#pragma unroll
+        for (int h = 1; h < G; ++h) mine = (lane == h) ? mb[h] : mine;
+        if (lane < G) xw[lane] = mine;
+        asm volatile("bar.sync %0, 64;" :: "r"(1 + pair) : "memory");
+#pragma unroll
+        for (int h = 0; h < G; ++h) mb[h] = fmaxf(mb[h], xr[h]);
+      }
+      uint8_t* pb0 = smem + sm.pb + (kTwoPBufs ? (i & 1) : st) * 2 * PBUF + (half * 4 + (lane >> 3)) * LBO_P + (lane & 7) * 2;   // token `tok`, row 0, hi
       float ls[G];
 #pragma unroll
       for (int h = 0; h < G; ++h) {
-        const float p0 = (v0 && mb[h] != kNegInf) ? fast_exp2(s0[h] - mb[h]) : 0.f;
-        const float p1 = (v1 && mb[h] != kNegInf) ? fast_exp2(s1[h] - mb[h]) : 0.f;
-        const __nv_bfloat16 h0 = __float2bfloat16_rn(p0), h1 = __float2bfloat16_rn(p1);
-        const __nv_bfloat16 l0 = __float2bfloat16_rn(p0 - __bfloat162float(h0)), l1 = __float2bfloat16_rn(p1 - __bfloat162float(h1));
+        const float p0 = (sv[h] != kNegInf) ? fast_exp2(sv[h] - mb[h]) : 0.f;
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(p0);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(p0 - __bfloat162float(h0));
         *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16) = h0;
-        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + 4 * LBO_P) = h1;              // token lane + 32: 4 chunks on
         *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF) = l0;
-        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF + 4 * LBO_P) = l1;
-        // the weight the tensor core really uses
-        ls[h] = (__bfloat162float(h0) + __bfloat162float(l0)) + (__bfloat162float(h1) + __bfloat162float(l1));
+        ls[h] = __bfloat162float(h0) + __bfloat162float(l0);  // the weight the tensor core really uses
       }
-      if (vmask != ~0ull) {                                   // masked V rows may hold NaN: 0 * NaN would poison P~V
+      if (vmask != ~0ull && !v0) {                            // masked V rows may hold NaN: 0 * NaN would poison P~V
         uint4* vr = reinterpret_cast<uint4*>(smem + sm.ring + st * kStageBytes + 2 * kBoxBytes);
-        if (!v0) {
 #pragma unroll
-          for (int c = 0; c < 8; ++c) { vr[lane * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[lane * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
-        }
-        if (!v1) {
-#pragma unroll
-          for (int c = 0; c < 8; ++c) { vr[(lane + 32) * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[(lane + 32) * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
-        }
+        for (int c = 0; c < 8; ++c) { vr[tok * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[tok * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
       }
-      // block sum per head: lane l ends up with the total of head head_of_lane32(l)
+      // sum of this half's weights per head: lane l ends up with the total of head head_of_lane32(l)
       Reduce32<G, 16>::run(ls, lane);
       {
         const int hh = head_of_lane32<G>(lane);
         float mine = mb[0];
 #pragma unroll
         for (int h = 1; h < G; ++h) mine = (hh == h) ? mb[h] : mine;
-        IterSlot& slot = slots[i & (kIterSlots - 1)];
-        if ((lane & (32 / G - 1)) == 0) { slot.mref[hh] = mine; slot.lsum[hh] = ls[0]; }
+        float* slot = slots + (i % kIterN) * 3 * G;
+        if ((lane & (32 / G - 1)) == 0) { if (half == 0) slot[hh] = mine; slot[(1 + half) * G + hh] = ls[0]; }
       }
       fence_proxy_async();                                    // P^T (and V fixes) visible to the tensor core
       mbar_arrive(bar(sm.pfull0 + st));
       if (q == 0 && lane == 0) TC_TRACE(trx, 9, i, 0);
-      st += NS; while (st >= S) st -= S;
+      st += 2; while (st >= S) st -= S;
     }
   } else if (warp < kWarpFold0 + 4) {
     // ===================================================== A5 / A6: publish step summaries, merge P~V_t
@@ -627,25 +634,28 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     };
     // merge block i (its P~V_t is relative to its own block maximum) into the running state
     auto fold = [&](int i) {
+      if (tid == 0) TC_TRACE(trf, 20, i, 0);
       tc_fence_after();
       float pv[G], pvl[G];
       tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN, pv);
       tmem_ld<G>(tmem_PV + tlane + (i & (NP - 1)) * kUmmaN + 8, pvl);
       tmem_ld_wait();
+      if (tid == 0) TC_TRACE(trf, 21, i, 0);
 #pragma unroll
       for (int h = 0; h < G; ++h) pv[h] += pvl[h];            // hi + lo halves of p
-      const IterSlot& sl = slots[i & (kIterSlots - 1)];
+      const float* sl = slots + (i % kIterN) * 3 * G;
 #pragma unroll
-      for (int h = 0; h < G; ++h) {
-        const float mr = sl.mref[h];
-        if (mr != kNegInf) {                                  // a block with no valid token changes nothing
-          const float mn = fmaxf(m_tot[h], mr);
-          const float a = fast_exp2(m_tot[h] - mn), bb = fast_exp2(mr - mn);
-          acc[h] = fmaf(a, acc[h], bb * pv[h]);
-          l_tot[h] = fmaf(a, l_tot[h], bb * sl.lsum[h]);
-          m_tot[h] = mn;
-        }
+      for (int h = 0; h < G; ++h) {                           // branch-free, so that the heads' chains overlap
+        const float mr = sl[h];
+        const bool some = mr != kNegInf;                      // a block with no valid token changes nothing
+        const float mn = fmaxf(m_tot[h], mr);
+        const float a = (m_tot[h] == mn) ? 1.f : fast_exp2(m_tot[h] - mn);
+        const float bb = some ? fast_exp2(mr - mn) : 0.f;
+        acc[h] = some ? fmaf(a, acc[h], bb * pv[h]) : acc[h];
+        l_tot[h] = some ? fmaf(a, l_tot[h], bb * (sl[G + h] + sl[2 * G + h])) : l_tot[h];
+        m_tot[h] = mn;
       }
+      if (tid == 0) TC_TRACE(trf, 22, i, 0);
       release_pv(i);
       if (tid == 0) TC_TRACE(trf, 5, i, item_step(item_t[i % kItemT]));
     };
@@ -657,52 +667,80 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     } else {
       int pub = 0, fld = 0;
       bool pub_ready = false;                                 // P~V of block `pub` is complete in tensor memory
+      int t_fld = 0, t_pub = 0;                               // steps of items fld (valid while fld < pub) and pub (valid while pub_ready)
+#ifdef ART_TRACE
+      long long clk_acc[6] = {0, 0, 0, 0, 0, 0}; int clk_cnt[6] = {0, 0, 0, 0, 0, 0};
+      if (TC_DBG(64)) trf.region = nullptr;
+#endif
+      // the thread that ships (m_blk, block sum) of a step: not one of warp 0's, whose lanes ship probe values first
+      const bool ml_thread = (tid == 97);
       while (fld < n_lim) {
-        const int ntot = ld_volatile_s32(a_ntotal);
+        TC_CLK(c0);
+        const int2 cn = ld_ctrl_ntotal(a_ctrl);
+        const int c = cn.x, ntot = cn.y;
         if (fld >= ntot) break;
-        const int c = ld_ctrl_relaxed(a_ctrl);
         // ---- merge the oldest unfolded block once the decision for the steps before it is known; one that
         //      lies beyond t* is dropped (its tensor-memory slot is released, nothing is merged)
         if (fld < pub) {
-          const int tf = item_step(item_t[fld % kItemT]);
-          if (c < 0 && tf > -c) { release_pv(fld); ++fld; continue; }
-          if (c < 0 || c >= tf - 1) { fold(fld); ++fld; continue; }
+          if (c < 0 && t_fld > -c) { release_pv(fld); ++fld; t_fld = item_step(item_t[fld % kItemT]); continue; }
+          if (c < 0 || c >= t_fld - 1 || TC_DBG(1)) {
+            TC_CLK(c1); fold(fld); ++fld; t_fld = item_step(item_t[fld % kItemT]); TC_CLK(c2); TC_ACC(0, c0, c1); TC_ACC(1, c1, c2);
+            continue;
+          }
         }
+        TC_CLK(c3);
         // ---- publish the summary of the next finished block (never waits for a decision on itself)
         if (pub < ntot && pub < n_lim && pub - fld < NP) {
-          const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
-          const uint32_t par = (pub / NP) & 1;
-          if (!pub_ready) { pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par); if (pub_ready && tid == 0) TC_TRACE(trf, 7, pub, 0); }
+          if (!pub_ready) {
+            const uint32_t pvb = bar(sm.pvfull0 + (pub & (NP - 1)));
+            const uint32_t par = (pub / NP) & 1;
+            pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
+            if (pub_ready) { t_pub = item_step(item_t[pub % kItemT]); if (tid == 0) TC_TRACE(trf, 7, pub, 0); }
+          }
+          TC_CLK(c4);
           if (pub_ready && c < 0) { ++pub; pub_ready = false; continue; }   // fired: an unpublished step lies beyond t*
-          const int t = pub_ready ? item_step(item_t[pub % kItemT]) : 0;
-          if (pub_ready && c >= t - M) {                      // mailbox slot free: step t - M has been scanned
+          if (pub_ready && (c >= t_pub - M || TC_DBG(4))) {   // mailbox slot free: step t - M has been scanned
+            const int t = t_pub;
             const int slot_i = (t - 1) & (M - 1);
+            const uint32_t row0 = mapa(sbase + sm.mbox + static_cast<uint32_t>(slot_i) * kSummaryBytes, 0);
+            const uint32_t mb = mapa(bar(sm.mbox0 + slot_i), 0);
             tc_fence_after();
             float pv[G], pvl[G];
             tmem_ld<G>(tmem_PV + tlane + (pub & (NP - 1)) * kUmmaN, pv);
             tmem_ld<G>(tmem_PV + tlane + (pub & (NP - 1)) * kUmmaN + 8, pvl);
+            if (ml_thread) {                                  // (overlaps the tensor-memory loads)
+              const float* sl = slots + (pub % kIterN) * 3 * G;
+              float ml[2 * G];
+#pragma unroll
+              for (int h = 0; h < G; ++h) { ml[h] = sl[h]; ml[G + h] = sl[G + h] + sl[2 * G + h]; }
+              st_async_vec<G>(row0, ml, mb);
+              st_async_vec<G>(row0 + G * 4u, ml + G, mb);
+            }
             tmem_ld_wait();
+            if (tid == 0) TC_TRACE(trf, 23, pub, 0);
 #pragma unroll
             for (int h = 0; h < G; ++h) pv[h] += pvl[h];
-            const IterSlot& sl = slots[pub & (kIterSlots - 1)];
-            const uint32_t row0 = mapa(sbase + sm.mbox + static_cast<uint32_t>(slot_i) * kSummaryBytes, 0);
-            const uint32_t mb = mapa(bar(sm.mbox0 + slot_i), 0);
             if (MODE == 2 || (d & 3) == 0) {
               const int pi = (MODE == 2) ? d : (d >> 2);      // probe coordinate k*(d/32)  (R1)
               st_async_vec<G>(row0 + (2 + pi) * G * 4u, pv, mb);
             }
-            if (d == 1) {
-              float ml[2 * G];
-#pragma unroll
-              for (int h = 0; h < G; ++h) { ml[h] = sl.mref[h]; ml[G + h] = sl.lsum[h]; }
-              st_async_vec<G>(row0, ml, mb);
-              st_async_vec<G>(row0 + G * 4u, ml + G, mb);
-            }
-            if (tid == 0) TC_TRACE(trf, 4, pub, t);
+            if (tid == 0) { TC_TRACE(trf, 4, pub, t); TC_TRACE(trf, 13, t, c < 0 ? 0 : c); }
+            if (fld == pub) t_fld = t;
             ++pub; pub_ready = false;
+            TC_CLK(c5); TC_ACC(2, c0, c3); TC_ACC(3, c3, c4); TC_ACC(4, c4, c5);
+            continue;
           }
         }
+        TC_CLK(c6); TC_ACC(5, c0, c6);
+        // nothing to do yet: do not take issue slots from the warps this one shares its scheduler with
+        if (p.fold_sleep > 0) __nanosleep(p.fold_sleep);
       }
+#ifdef ART_TRACE
+      if (tid == 0 && p.trace && TC_DBG(64)) {
+        unsigned long long* acc = reinterpret_cast<unsigned long long*>(p.trace + 64);
+        for (int k = 0; k < 6; ++k) { atomicAdd(acc + 2 * k, static_cast<unsigned long long>(clk_acc[k])); atomicAdd(acc + 2 * k + 1, static_cast<unsigned long long>(clk_cnt[k])); }
+      }
+#endif
     }
   } else if (ART && warp == kWarpScan && rank == 0) {
     // ===================================================== A6 + A7 + A9: Algorithm 1 over step summaries
@@ -718,6 +756,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     while (t <= Tn) {
       const int i0 = t - 1;                                   // 0-based step index of the batch head
       mbar_wait(bar(sm.mbox0 + (i0 & (M - 1))), (i0 >> mshift) & 1);
+      if (lane == 0) TC_TRACE(trs, 14, t, 0);
       // how many of the following steps have arrived as well (lane k probes step t + k)
       int n = 1;
       {
@@ -729,7 +768,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         n = n > kScanBatch ? kScanBatch : n;
         __syncwarp();                                         // the probing lane's acquire covers the whole warp
       }
-      const int fired = sc.batch(n, lane, p.tau, p.phi, p.patience,
+      const int fired = TC_DBG(2) ? -1 : sc.batch(n, lane, p.tau, p.phi, p.patience,
         [&](int k, bool live, float& mt, float& lt) {
           const uint32_t a = mb_lane + static_cast<uint32_t>((i0 + k) & (M - 1)) * kSummaryBytes;
           const float m_ = lds_f32(a), l_ = lds_f32(a + G * 4u);     // a slot that is not part of the batch
