@@ -92,9 +92,8 @@ typedef struct art_desc {
                                   as many as fit the GPU at once; each takes groups from a queue and its CTAs claim
                                   steps of whichever of the cluster's open groups has work left (needs `workspace`).
                                   A detector-on call with split < 0 runs static clusters of the library's choice.
-                                  0 = the library decides: static clusters sized so that groups x CTAs fill the GPU,
-                                  except for detector-off BF16 calls with more groups than one-CTA clusters fit at
-                                  once (many short groups), which use persistent clusters when a workspace is given.
+                                  0 = the library decides: static clusters sized so that groups x CTAs fill the GPU
+                                  (persistent clusters run only when split < 0 asks for them).
                                   Any value gives the same stop_block as the sequential algorithm. */
   int32_t q_len;               /* m: query tokens per sequence (speculative decode, the tail of a chunked
                                   prefill); 0 or 1 = plain decode.  The m tokens are the LAST m positions of the

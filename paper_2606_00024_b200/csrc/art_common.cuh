@@ -42,9 +42,8 @@ struct Params {
   float tau, phi;
   int32_t patience;
   int32_t stages, mbox_slots;
-  int32_t dyn;                                       // bf16 cluster kernel: steps claimed at run time instead of dealt round-robin
+  int32_t dyn;                                       // 1 in the persistent-cluster kernel (steps claimed at run time); static clusters deal round-robin
   int32_t run_ahead;                                 // bf16 cluster kernel, detector on: loads of step t are issued once step t - run_ahead is decided (0 = no limit)
-  int32_t fold_sleep;                                // bf16 cluster kernel, detector on: ns a fold warp sleeps when it can neither publish nor merge (0 = spin)
 #ifdef ART_TRACE
   uint8_t* trace;
   int32_t dbg;                                       // timing experiments of the trace build (ART_DBG): results are NOT exact

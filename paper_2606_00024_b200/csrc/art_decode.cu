@@ -300,13 +300,6 @@ static int static_run_ahead(int C, int stages) {
   return C * (stages + 3) + 4;
 }
 
-// static bf16 clusters, detector on: how long a fold warp that can neither publish nor merge sleeps before it looks again
-// (a warp that polls takes issue slots from the softmax, MMA-issue and scan warps of its scheduler).  ART_FOLD_SLEEP overrides.
-static int fold_sleep_ns() {
-  static const int env = [] { const char* e = getenv("ART_FOLD_SLEEP"); return e ? atoi(e) : -1; }();
-  return env >= 0 ? env : 0;
-}
-
 // workspace of the persistent-cluster kernel: one partial state (m, l, acc) per (group, CTA of a cluster)
 static size_t pc_part_bytes(int groups, int G) {
   return static_cast<size_t>(groups) * pc::kMaxCL * static_cast<size_t>(G * (tc::kD + 2)) * 4u;
@@ -327,9 +320,10 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   const int PW = mode == 2 ? d->head_dim : 32;
   const bool tensor_core = d->dtype == ART_DTYPE_BF16;
   // Static clusters are the default: every group streams from the first cycle and, with the detector on, the decision
-  // loop of a group never leaves its cluster.  When the detector is off and the groups do not even fit one 2-CTA
-  // cluster each (many short groups: configs[3]), persistent clusters that pull groups from their queue avoid the
-  // waves of short-lived CTAs; they need the caller's workspace.
+  // loop of a group never leaves its cluster.  Persistent clusters that pull groups from a queue (detector off; they
+  // need the caller's workspace) run only when split < 0 asks for them: since the S-MMA / P.V-MMA operand traffic was
+  // halved, waves of one-CTA static clusters are as fast on many short groups (configs[3]: 340 / 330 us against
+  // 338 / 336 us).
   Route rt = route_of_split(d);
   if (rt.persistent && mode != 0) rt = {false, 0};         // persistent clusters exist for the detector-off path only
   const size_t pc_need = tensor_core ? pc_part_bytes(groups, G) : 0;
@@ -338,7 +332,6 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
   if (!rt.persistent) {
     int rc = choose_split(d, mode, rt.want, &C_static);
     if (rc != ART_OK) return rc;
-    if (tensor_core && d->split == 0 && mode == 0 && C_static == 1 && ws_ok) rt = {true, 0};
   }
   const bool persistent = rt.persistent;
 
@@ -397,14 +390,12 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
     const int C = C_static;
     const LaunchPlan pl = plan_for(tensor_core, G, PW, mode != 0, C);
     p.stages = pl.stages; p.mbox_slots = pl.mslots;
-    // static bf16 clusters: with the detector on, steps are claimed at run time for clusters of 2-4 (measured in round 1)
-    p.dyn = (tensor_core && mode != 0 && C >= 2 && C <= 4) ? 1 : 0;
+    p.dyn = 0;                                               // static clusters deal their steps round-robin
     p.run_ahead = (tensor_core && mode != 0) ? static_run_ahead(C, pl.stages) : 0;
-    p.fold_sleep = fold_sleep_ns();
     if (tensor_core) {
 #ifdef ART_TRACE
       if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
-      { const char* e = getenv("ART_DBG"); p.dbg = e ? atoi(e) : 0; if (p.dbg & 8) p.dyn = 0; if (p.dbg & 16) p.dyn = (mode != 0); }
+      { const char* e = getenv("ART_DBG"); p.dbg = e ? atoi(e) : 0; }
 #endif
       CUtensorMap tmK, tmV;
       if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
@@ -648,7 +639,6 @@ static int query_shape(const art_desc_t* desc, int art_on, int* C_out, int* NC_o
   if (!rt.persistent) {
     rc = art::choose_split(desc, mode, rt.want, &C);
     if (rc != ART_OK) return rc;
-    if (desc->dtype == ART_DTYPE_BF16 && desc->split == 0 && mode == 0 && C == 1) rt = {true, 0};
   } else if (mode != 0) {                                  // persistent clusters exist for the detector-off path only
     rt = {false, 0};
     rc = art::choose_split(desc, mode, 0, &C);

@@ -55,7 +55,7 @@ __device__ __forceinline__ int item_kind(int meta) { return (meta >> 6) & 3; }
 struct HomeInfo { unsigned long long done; int group, T, gen, loaded; unsigned joined; int pad; };   // home CTA: one per local slot
 
 struct SmemMapP {
-  uint32_t qb, pb, slots, items, hinfo, board, bars, misc, ring, total;
+  uint32_t qb, pb, slots, xch, items, hinfo, board, bars, misc, ring, total;
   uint32_t full0, empty0, pfull0, sfull0, sfree0, pvfull0, pvfree0, done0, nbars;
 };
 
@@ -64,7 +64,8 @@ __host__ __device__ inline SmemMapP make_smem_map_p(int G, int stages) {
   uint32_t off = 0;
   m.qb = off; off += 2u * kQBytes;
   m.pb = off; off += static_cast<uint32_t>(stages) * 2u * p_buf_bytes(G);
-  m.slots = off; off += kIterSlots * static_cast<uint32_t>(2 * G) * 4u;           // per item: m_blk[G], block sum[G]
+  m.slots = off; off += kIterSlots * static_cast<uint32_t>(3 * G) * 4u;           // per item: m_blk[G], block sum of tokens 0-31 [G], of tokens 32-63 [G]
+  m.xch = off; off += 8u * G * 4u;                                                // block maxima of the two token halves: [pair][parity][half][G]
   m.items = off; off += kItemsRing * static_cast<uint32_t>(sizeof(Item));
   off = (off + 15u) & ~15u;
   m.hinfo = off; off += 2u * static_cast<uint32_t>(sizeof(HomeInfo));
@@ -156,7 +157,8 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
   if ((sbase & 1023u) != 0u) __trap();
   const uint32_t bars = sbase + sm.bars;
   auto bar = [&](uint32_t idx) { return bars + idx * 8u; };
-  float* slots = reinterpret_cast<float*>(smem + sm.slots);   // [item & 15][2 G]: block maximum (log2 domain), block sum
+  float* slots = reinterpret_cast<float*>(smem + sm.slots);   // [item & 15][3 G]: block maximum (log2 domain), block sums of the two token halves
+  float* xch = reinterpret_cast<float*>(smem + sm.xch);
   volatile Item* items = reinterpret_cast<volatile Item*>(smem + sm.items);
   const uint32_t a_misc = sbase + sm.misc;
 
@@ -176,8 +178,8 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
 
   // ---- one-time setup
   if (tid == 0) {
-    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 32); }
-    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 1); }
+    for (int s = 0; s < S; ++s) { mbar_init(bar(sm.full0 + s), 1); mbar_init(bar(sm.empty0 + s), 1); mbar_init(bar(sm.pfull0 + s), 64); }
+    for (int s = 0; s < NS; ++s) { mbar_init(bar(sm.sfull0 + s), 1); mbar_init(bar(sm.sfree0 + s), 2); }
     for (int s = 0; s < NP; ++s) { mbar_init(bar(sm.pvfull0 + s), 1); mbar_init(bar(sm.pvfree0 + s), 4); }
     mbar_init(bar(sm.done0), 1); mbar_init(bar(sm.done0 + 1), 1);
     st_volatile_s32(a_misc + kMFlag, 0);
@@ -205,7 +207,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
   cluster_sync_all();                                        // boards and barriers of every CTA are live
   tc_fence_after();
   const uint32_t tmem_base = static_cast<uint32_t>(ld_volatile_s32(a_misc + kMTmem));
-  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kSCols;
+  const uint32_t tmem_S = tmem_base, tmem_PV = tmem_base + NS * kSCols1;
 
   // fold warps: output coordinate and running (un-normalised) partial state of the current visit
   const int fq = warp & 3;
@@ -457,14 +459,13 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
         if (kind == ITEM_DATA) {
           tc_fence_after();
           const uint32_t qb = sbase + sm.qb + item_q(meta) * kQBytes;
-          const uint32_t kt = sbase + sm.ring + st * kStageBytes - q * 4096;
-          const uint32_t dcol = tmem_S + q * kSCols;
+          // one M128 MMA per k-step: tokens on lanes 0-63 (even items) or 64-127 (odd items), see art_decode_tc.cuh
+          const uint32_t kt = sbase + sm.ring + st * kStageBytes - (i & 1) * kBoxBytes;
+          const uint32_t dcol = tmem_S + q * kSCols1;
 #pragma unroll
           for (int ks = 0; ks < 8; ++ks) {
             const uint32_t ka = kt + (ks >> 2) * kBoxBytes + (ks & 3) * 32;
-            const uint64_t bq = dQ | desc_addr(qb + ks * 2 * kQLbo);
-            umma_bf16(dcol, dK | desc_addr(ka), bq, kIdescS, ks > 0);
-            umma_bf16(dcol + kUmmaN, dK | desc_addr(ka + 4096), bq, kIdescS, ks > 0);
+            umma_bf16(dcol, dK | desc_addr(ka), dQ | desc_addr(qb + ks * 2 * kQLbo), kIdescS, ks > 0);
           }
         }
         umma_commit(bar(sm.sfull0 + q));
@@ -502,78 +503,74 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
       mbar_wait(bar(sm.done0 + 1), 0);
     }
   } else if (warp >= kWarpSoftmax0 && warp < kWarpSoftmax0 + 4) {
-    // ===================================================== A4: block-local softmax, two tokens per thread
-    const int q = warp - kWarpSoftmax0;
-    const uint32_t taddr = tmem_S + q * kSCols + (static_cast<uint32_t>(q * 32) << 16);
-    int st = q % S;
-    for (int i = q;; i += NS) {
-      mbar_wait(bar(sm.sfull0 + q), (i / NS) & 1);
+    // ===================================================== A4: block-local softmax, one token per thread, two warps per item
+    const int q = warp - kWarpSoftmax0;                       // TMEM lane quadrant
+    const int pair = q >> 1, half = q & 1;                    // the pair owns items i = pair (mod 2); this warp tokens 32 half + lane
+    const int tok = half * 32 + lane;
+    const uint32_t tq = static_cast<uint32_t>(q * 32) << 16;
+    int st = pair % S;
+    for (int i = pair;; i += 2) {
+      const int sslot = i & (NS - 1);
+      mbar_wait(bar(sm.sfull0 + sslot), (i / NS) & 1);
       const int kind = item_kind(items[i % kItemsRing].meta);
       if (kind == ITEM_END) {
-        // the END item that owns a stage is the first of the four; only its warp hands it on to the P.V issuer
+        // the END item that owns a stage is the first of the run; only its pair hands it on to the P.V issuer
         if (item_kind(items[(i + kItemsRing - 1) % kItemsRing].meta) != ITEM_END || i == 0) mbar_arrive(bar(sm.pfull0 + st));
         break;
       }
       if (kind != ITEM_DATA) {                               // a marker: nothing to compute
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+        if (lane == 0) mbar_arrive(bar(sm.sfree0 + sslot));
         mbar_arrive(bar(sm.pfull0 + st));
-        st += NS; while (st >= S) st -= S;
+        st += 2; while (st >= S) st -= S;
         continue;
       }
       tc_fence_after();
-      float s0[G], s1[G];
-      tmem_ld<G>(taddr, s0);
-      tmem_ld<G>(taddr + kUmmaN, s1);
+      float sv[G];
+      tmem_ld<G>(tmem_S + sslot * kSCols1 + tq, sv);
       tmem_ld_wait();
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(sm.sfree0 + q));
+      if (lane == 0) mbar_arrive(bar(sm.sfree0 + sslot));
       const unsigned long long vmask = items[i % kItemsRing].mask;
-      const bool v0 = (vmask >> lane) & 1ull, v1 = (vmask >> (lane + 32)) & 1ull;
+      const bool v0 = (vmask >> tok) & 1ull;
       float mb[G];
       int ec = 0;
       if constexpr (MT) ec = items[i % kItemsRing].tcode >> kItemShift;
-      if (MT && ec != 0) {                                    // R15: the most recent tokens are cut row by row
 #pragma unroll
-        for (int h = 0; h < G; ++h) {
-          const int lim = ec - static_cast<int>((p.cuts >> (4 * h)) & 15u);
-          s0[h] = (v0 && lane < lim) ? s0[h] * p.scale_log2 : kNegInf;
-          s1[h] = (v1 && lane + 32 < lim) ? s1[h] * p.scale_log2 : kNegInf;
-          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
-        }
-      } else {
-#pragma unroll
-        for (int h = 0; h < G; ++h) {
-          s0[h] = v0 ? s0[h] * p.scale_log2 : kNegInf;        // masked tokens: weight 0 (R8); their K may be NaN
-          s1[h] = v1 ? s1[h] * p.scale_log2 : kNegInf;
-          mb[h] = warp_max_f32(fmaxf(s0[h], s1[h]));
-        }
+      for (int h = 0; h < G; ++h) {
+        bool vis = v0;                                        // masked tokens: weight 0 (R8); their K may be NaN
+        if (MT && ec != 0) vis = vis && tok < ec - static_cast<int>((p.cuts >> (4 * h)) & 15u);   // R15: causal cut row by row
+        sv[h] = vis ? sv[h] * p.scale_log2 : kNegInf;
+        mb[h] = warp_max_f32(sv[h]);
       }
-      uint8_t* pb0 = smem + sm.pb + st * 2 * PBUF + (lane >> 3) * LBO_P + (lane & 7) * 2;
+      {
+        // block maximum over the two halves (shared memory + the pair's named barrier; double-buffered by item parity)
+        float* xw = xch + (((pair * 2 + ((i >> 1) & 1)) * 2) + half) * G;
+        const float* xr = xch + (((pair * 2 + ((i >> 1) & 1)) * 2) + (half ^ 1)) * G;
+        float mine = mb[0];
+#pragma unroll
+        for (int h = 1; h < G; ++h) mine = (lane == h) ? mb[h] : mine;
+        if (lane < G) xw[lane] = mine;
+        asm volatile("bar.sync %0, 64;" :: "r"(2 + pair) : "memory");   // named barriers 2, 3 (0: __syncthreads, 1: fold warps of the persistent kernel)
+#pragma unroll
+        for (int h = 0; h < G; ++h) mb[h] = fmaxf(mb[h], xr[h]);
+      }
+      uint8_t* pb0 = smem + sm.pb + st * 2 * PBUF + (half * 4 + (lane >> 3)) * LBO_P + (lane & 7) * 2;
       float ls[G];
 #pragma unroll
       for (int h = 0; h < G; ++h) {
-        const float p0 = (v0 && mb[h] != kNegInf) ? fast_exp2(s0[h] - mb[h]) : 0.f;
-        const float p1 = (v1 && mb[h] != kNegInf) ? fast_exp2(s1[h] - mb[h]) : 0.f;
-        const __nv_bfloat16 h0 = __float2bfloat16_rn(p0), h1 = __float2bfloat16_rn(p1);
-        const __nv_bfloat16 l0 = __float2bfloat16_rn(p0 - __bfloat162float(h0)), l1 = __float2bfloat16_rn(p1 - __bfloat162float(h1));
+        const float p0 = (sv[h] != kNegInf) ? fast_exp2(sv[h] - mb[h]) : 0.f;
+        const __nv_bfloat16 h0 = __float2bfloat16_rn(p0);
+        const __nv_bfloat16 l0 = __float2bfloat16_rn(p0 - __bfloat162float(h0));
         *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16) = h0;
-        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + 4 * LBO_P) = h1;
         *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF) = l0;
-        *reinterpret_cast<__nv_bfloat16*>(pb0 + h * 16 + PBUF + 4 * LBO_P) = l1;
-        ls[h] = (__bfloat162float(h0) + __bfloat162float(l0)) + (__bfloat162float(h1) + __bfloat162float(l1));
+        ls[h] = __bfloat162float(h0) + __bfloat162float(l0);
       }
-      if (vmask != ~0ull) {                                   // masked V rows may hold NaN: 0 * NaN would poison P~V
+      if (vmask != ~0ull && !v0) {                            // masked V rows may hold NaN: 0 * NaN would poison P~V
         uint4* vr = reinterpret_cast<uint4*>(smem + sm.ring + st * kStageBytes + 2 * kBoxBytes);
-        if (!v0) {
 #pragma unroll
-          for (int c = 0; c < 8; ++c) { vr[lane * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[lane * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
-        }
-        if (!v1) {
-#pragma unroll
-          for (int c = 0; c < 8; ++c) { vr[(lane + 32) * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[(lane + 32) * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
-        }
+        for (int c = 0; c < 8; ++c) { vr[tok * 8 + c] = make_uint4(0u, 0u, 0u, 0u); vr[tok * 8 + c + kBoxBytes / 16] = make_uint4(0u, 0u, 0u, 0u); }
       }
       Reduce32<G, 16>::run(ls, lane);
       {
@@ -581,12 +578,12 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
         float mine = mb[0];
 #pragma unroll
         for (int h = 1; h < G; ++h) mine = (hh == h) ? mb[h] : mine;
-        float* slot = slots + (i & (kIterSlots - 1)) * 2 * G;
-        if ((lane & (32 / G - 1)) == 0) { slot[hh] = mine; slot[G + hh] = ls[0]; }
+        float* slot = slots + (i & (kIterSlots - 1)) * 3 * G;
+        if ((lane & (32 / G - 1)) == 0) { if (half == 0) slot[hh] = mine; slot[(1 + half) * G + hh] = ls[0]; }
       }
       fence_proxy_async();
       mbar_arrive(bar(sm.pfull0 + st));
-      st += NS; while (st >= S) st -= S;
+      st += 2; while (st >= S) st -= S;
     }
   } else if (warp < kWarpFold0 + 4) {
     // ===================================================== A5 / A6 / A8 / A9: publish summaries, merge P~V_t, flush, combine
@@ -612,7 +609,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
       tmem_ld_wait();
 #pragma unroll
       for (int h = 0; h < G; ++h) pv[h] += pvl[h];            // hi + lo halves of p
-      const float* sl = slots + (i & (kIterSlots - 1)) * 2 * G;
+      const float* sl = slots + (i & (kIterSlots - 1)) * 3 * G;
 #pragma unroll
       for (int h = 0; h < G; ++h) {
         const float mr = sl[h];
@@ -620,7 +617,7 @@ art_decode_pc_kernel(const PcParams pp, const __grid_constant__ CUtensorMap tmK,
           const float mn = fmaxf(m_tot[h], mr);
           const float a = fast_exp2(m_tot[h] - mn), bb = fast_exp2(mr - mn);
           acc[h] = fmaf(a, acc[h], bb * pv[h]);
-          l_tot[h] = fmaf(a, l_tot[h], bb * sl[G + h]);
+          l_tot[h] = fmaf(a, l_tot[h], bb * (sl[G + h] + sl[2 * G + h]));
           m_tot[h] = mn;
         }
       }

@@ -121,7 +121,7 @@ __host__ __device__ inline SmemMap make_smem_map(int G, int PW, int stages, int 
   m.total = off;
   return m;
 }
-constexpr uint32_t kCtrl = 0, kNTotal = 4, kLoaded = 8, kTmemPtr = 12, kNext = 16;   // (ctrl, n_total) are read as one 8-byte word
+constexpr uint32_t kCtrl = 0, kNTotal = 4, kLoaded = 8, kTmemPtr = 12;   // (ctrl, n_total) are read as one 8-byte word
 
 // An entry of the item ring: the step number in the low 24 bits and, for multi-token queries (R15), the causal
 // code of the step's block above them: e = L - 64 * blk (tokens of the sequence from the start of this block on)
@@ -286,7 +286,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
   const Trav tr = make_trav(p, b, g, L);
   const int Tn = tr.T;
   const int n_c = (Tn > rank) ? (Tn - rank + C - 1) / C : 0;   // steps of this CTA when they are dealt round-robin
-  const int n_lim = p.dyn ? 0x7fffffff : n_c;                 // items this CTA will process, if known up front
+  const int n_lim = n_c;                                      // items this CTA will process unless Algorithm 1 fires first
   constexpr int kItemT = item_ring(G, MODE == 1);
   int* item_t = reinterpret_cast<int*>(smem + sm.items);      // step number of item i (i mod kItemT)
   auto item_step = [](int v) { return MT ? (v & kItemStep) : v; };
@@ -309,7 +309,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       }
     }
     st_volatile_s32(a_ctrl, 0); st_volatile_s32(a_loaded, 0);
-    st_volatile_s32(sbase + sm.misc + kNext, 0); st_volatile_s32(a_ntotal, 0x7fffffff); st_volatile_s32(sbase + sm.misc + 20, 0);
+    st_volatile_s32(a_ntotal, 0x7fffffff); st_volatile_s32(sbase + sm.misc + 20, 0);
     fence_mbar_init();
   }
   if (warp == kWarpMmaPV) tmem_alloc(a_tmem, kTmemCols);
@@ -350,8 +350,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     }
   };
   // Every issued item runs through all roles (one beyond t* is dropped by the fold warps); a wait can only fail
-  // once the producer has issued its last item (known up front, n_lim, unless steps are claimed at run time
-  // or Algorithm 1 fires).
+  // once the producer has issued its last item (n_lim, fewer if Algorithm 1 fires).
   auto wait_item = [&](uint32_t baddr, uint32_t parity, int i) -> bool {
     if constexpr (!ART) { mbar_wait(baddr, parity); return true; }          // detector off: every item arrives
     while (!mbar_try_wait(baddr, parity)) { if (i >= ld_volatile_s32(a_ntotal)) return false; }
@@ -370,67 +369,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     int it_issued = 0, loaded = 0, stage = 0;
     TC_TRACE_INIT(trc, 0);
     uint32_t ph = 0;                                          // (it / S) & 1
-    if (p.dyn) {
-      // ---- steps CLAIMED at run time from a counter in the leader's shared memory: a CTA that shares its SM takes
-      //      fewer steps than one that has an SM to itself, and nobody waits at the mailbox window for a slower CTA
-      int it = 0;
-      const uint32_t a_next = mapa(sbase + sm.misc + kNext, 0); // the cluster's claim counter lives in the leader
-      auto claim = [&]() -> int {                               // next unclaimed step, 1-based
-        uint32_t r;
-        asm volatile("atom.relaxed.cluster.shared::cluster.add.u32 %0, [%1], 1;" : "=r"(r) : "r"(a_next) : "memory");
-        return static_cast<int>(r) + 1;
-      };
-      // resolve a claimed step: validity, token mask, page (the table lookup is left in flight)
-      auto resolve = [&](int t, bool& valid, unsigned long long& mask, int& page, int& ec) {
-        valid = t <= Tn && !beyond_stop(t);                     // exhausted, or beyond t* (A7: stop prefetching)
-        mask = 0ull; page = 0; ec = 0;
-        if (valid) {
-          const int blk = trav_block(tr, t);
-          mask = block_mask(p, L, blk);
-          if constexpr (MT) ec = causal_code(p, L, blk);
-          if (mask) page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
-        }
-      };
-      // claim -> page lookup -> TMA is software-pipelined: item A resolved, item B claimed, next claim issued
-      int tB = 0;
-      if (lane == 0) tB = claim();
-      int tA = __shfl_sync(0xffffffffu, tB, 0);
-      bool validA; unsigned long long maskA; int pageA, ecA;
-      resolve(tA, validA, maskA, pageA, ecA);
-      if (lane == 0) tB = claim();
-      while (validA) {
-        const int tN = __shfl_sync(0xffffffffu, tB, 0);
-        bool validB; unsigned long long maskB; int pageB, ecB;
-        resolve(tN, validB, maskB, pageB, ecB);
-        if (validB && lane == 0) tB = claim();
-        if (!may_issue(tA)) break;                             // (waits for step tA - run_ahead to be decided)
-        if (it >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);                  // slot released?
-        if (lane == 0) {
-          TC_TRACE(trc, 1, group, tA);
-          const uint32_t fb = bar(sm.full0 + stage);
-          const uint32_t dst = sbase + sm.ring + stage * kStageBytes;
-          item_t[it % kItemT] = tA | (ecA << kItemShift);
-          sinfo[stage] = maskA;
-          if (maskA == 0ull) {
-            mbar_arrive(fb);                                   // nothing to load: an all-masked step
-          } else {
-            int c1, c2;
-            if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = pageA * p.Hkv + g; }   // [page*Hkv + head][token][d]
-            else { c1 = g; c2 = pageA * kBlockTokens; }                           // [page*64 + token][head][d]
-            mbar_arrive_expect_tx(fb, kStageBytes);
-            tma_load_box(dst, &tmK, 0, c1, c2, fb);
-            tma_load_box(dst + kBoxBytes, &tmK, 64, c1, c2, fb);
-            tma_load_box(dst + 2 * kBoxBytes, &tmV, 0, c1, c2, fb);
-            tma_load_box(dst + 3 * kBoxBytes, &tmV, 64, c1, c2, fb);
-          }
-        }
-        if (maskA != 0ull) ++loaded;
-        ++it;
-        if (++stage == S) { stage = 0; ph ^= 1u; }
-        tA = tN; validA = validB; maskA = maskB; pageA = pageB; ecA = ecB;
-      }
-      it_issued = it;
-    } else {
+    {
       // ---- steps dealt round-robin: CTA c owns steps c+1, c+1+C, ...; 32 of them are resolved at a time
       auto step_of = [&](int i) { return i * C + rank + 1; };
       bool stop = false;
@@ -588,7 +527,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
 #pragma unroll
         for (int h = 1; h < G; ++h) mine = (lane == h) ? mb[h] : mine;
         if (lane < G) xw[lane] = mine;
-        asm volatile("bar.sync %0, 64;" :: "r"(1 + pair) : "memory");
+        asm volatile("bar.sync %0, 64;" :: "r"(2 + pair) : "memory");   // named barriers 2, 3 (0: __syncthreads, 1: fold warps of the persistent kernel)
 #pragma unroll
         for (int h = 0; h < G; ++h) mb[h] = fmaxf(mb[h], xr[h]);
       }
@@ -733,7 +672,6 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         }
         TC_CLK(c6); TC_ACC(5, c0, c6);
         // nothing to do yet: do not take issue slots from the warps this one shares its scheduler with
-        if (p.fold_sleep > 0) __nanosleep(p.fold_sleep);
       }
 #ifdef ART_TRACE
       if (tid == 0 && p.trace && TC_DBG(64)) {
