@@ -292,12 +292,12 @@ static unsigned long long* watchdog_word() {
 #endif
 
 // static bf16 clusters, detector on: how far the loads of a group may run ahead of its last decided step.  Every CTA of
-// the cluster keeps its ring full (stages) plus the blocks on their way through S-MMA / softmax / P.V / mailbox / scan.
+// the cluster keeps its ring full (stages) plus two blocks per CTA on their way through P.V / mailbox / scan (+ 4).
 // ART_RUNAHEAD overrides it for measurements (0 = no limit, the behaviour of round 1).
 static int static_run_ahead(int C, int stages) {
   static const int env = [] { const char* e = getenv("ART_RUNAHEAD"); return e ? atoi(e) : -1; }();
   if (env >= 0) return env;
-  return C * (stages + 3) + 4;
+  return C * (stages + 2) + 4;
 }
 
 // workspace of the persistent-cluster kernel: one partial state (m, l, acc) per (group, CTA of a cluster)
