@@ -618,7 +618,10 @@ def main():
                          "frac": achieved / peak, "traffic": traffic, "peak_kind": which,
                          "kernel": "art::tc::art_decode_tc_kernel<4, 1, false>",
                          "bytes_per_launch": ld * BLOCK_BYTES, "frac_of_nominal_8TBs": achieved / 8000.0,
-                         "read_only_ceiling_gbs": ceiling_gbs, "frac_of_read_only_ceiling": achieved / ceiling_gbs},
+                         "read_only_ceiling_gbs": ceiling_gbs, "frac_of_read_only_ceiling": achieved / ceiling_gbs,
+                         "note": "peak is the pool's measured COPY bandwidth (read + write); this kernel only reads, so "
+                                 "frac may exceed 1 -- frac_of_read_only_ceiling is against a read-only TMA stream "
+                                 "(art_hbm_read_probe over 4 GiB) timed in this run"},
             "art": {"on_us_per_step": us, "off_us_per_step": off["us_per_step"],
                     "off_gbs": off["gbs_processed"], "off_frac_of_peak": off["gbs_processed"] / peak,
                     "pinf_overhead": pinf["us_per_step"] / off["us_per_step"] - 1.0,

@@ -136,14 +136,14 @@ typedef struct art_thresholds {
  *                                                T if the criterion never fired
  *   workspace       DEVICE scratch, 256-B aligned, >= art_workspace_bytes(desc); only the persistent-cluster kernel
  *                   uses it (partial online-softmax states, [group][CTA of the cluster][G][d + 2] floats, written
- *                   before they are read: nothing needs zeroing).  May be NULL: split == 0 then stays on static
- *                   clusters, split < 0 on a detector-off call returns ART_ERR_WORKSPACE
+ *                   before they are read: nothing needs zeroing).  May be NULL unless split < 0 on a detector-off
+ *                   call (ART_ERR_WORKSPACE); split >= 0 runs static clusters, which need none
  *
  * seq_lens[b] == 0 or an empty list gives a zero output row and stop_block 0.
- * Reproducibility: stop_block is bit-deterministic for every schedule.  `out` is bit-reproducible when steps are
- * dealt statically (static clusters of 1 or > 4 CTAs, static clusters with the detector off); when CTAs claim steps at
- * run time (detector on with static clusters of 2-4, persistent clusters) which CTA folds which step depends on the
- * run and `out` agrees to fp32 rounding (<= 1e-5 relative) between runs.
+ * Reproducibility: stop_block is bit-deterministic for every schedule.  `out` is bit-reproducible with static
+ * clusters (steps are dealt round-robin, every CTA merges its steps in order, the partial states are combined in rank
+ * order); with persistent clusters CTAs claim steps at run time, which CTA folds which step depends on the run and
+ * `out` agrees to fp32 rounding (<= 1e-5 relative) between runs.
  * Device-side contents (page ids in range, list entries valid and distinct, seq_lens within the table) are not
  * validated by the release build; a library built with -DART_DEBUG runs a checking kernel before every launch that
  * records the first violation and traps (tests/test_gpu_debug_build.py).

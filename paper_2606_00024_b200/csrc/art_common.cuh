@@ -46,7 +46,6 @@ struct Params {
   int32_t run_ahead;                                 // bf16 cluster kernel, detector on: loads of step t are issued once step t - run_ahead is decided (0 = no limit)
 #ifdef ART_TRACE
   uint8_t* trace;
-  int32_t dbg;                                       // timing experiments of the trace build (ART_DBG): results are NOT exact
 #endif
 };
 

@@ -395,7 +395,6 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
     if (tensor_core) {
 #ifdef ART_TRACE
       if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
-      { const char* e = getenv("ART_DBG"); p.dbg = e ? atoi(e) : 0; }
 #endif
       CUtensorMap tmK, tmV;
       if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))

@@ -43,13 +43,7 @@ namespace tc {
 #ifdef ART_TRACE
 #define TC_TRACE_INIT(tr, role) Tracer tr; tr.init(p.trace, 0, role, reinterpret_cast<volatile int*>(smem + sm.misc + 20))
 #define TC_TRACE(tr, code, a, b) tr.ev(code, a, b)
-#define TC_DBG(bit) ((p.dbg & (bit)) != 0)
-#define TC_CLK(v) const long long v = clock64()
-#define TC_ACC(k, a, b) do { clk_acc[k] += (b) - (a); ++clk_cnt[k]; } while (0)
 #else
-#define TC_DBG(bit) false
-#define TC_CLK(v)
-#define TC_ACC(k, a, b)
 #define TC_TRACE_INIT(tr, role)
 #define TC_TRACE(tr, code, a, b)
 #endif
@@ -607,14 +601,9 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       int pub = 0, fld = 0;
       bool pub_ready = false;                                 // P~V of block `pub` is complete in tensor memory
       int t_fld = 0, t_pub = 0;                               // steps of items fld (valid while fld < pub) and pub (valid while pub_ready)
-#ifdef ART_TRACE
-      long long clk_acc[6] = {0, 0, 0, 0, 0, 0}; int clk_cnt[6] = {0, 0, 0, 0, 0, 0};
-      if (TC_DBG(64)) trf.region = nullptr;
-#endif
       // the thread that ships (m_blk, block sum) of a step: not one of warp 0's, whose lanes ship probe values first
       const bool ml_thread = (tid == 97);
       while (fld < n_lim) {
-        TC_CLK(c0);
         const int2 cn = ld_ctrl_ntotal(a_ctrl);
         const int c = cn.x, ntot = cn.y;
         if (fld >= ntot) break;
@@ -622,12 +611,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         //      lies beyond t* is dropped (its tensor-memory slot is released, nothing is merged)
         if (fld < pub) {
           if (c < 0 && t_fld > -c) { release_pv(fld); ++fld; t_fld = item_step(item_t[fld % kItemT]); continue; }
-          if (c < 0 || c >= t_fld - 1 || TC_DBG(1)) {
-            TC_CLK(c1); fold(fld); ++fld; t_fld = item_step(item_t[fld % kItemT]); TC_CLK(c2); TC_ACC(0, c0, c1); TC_ACC(1, c1, c2);
-            continue;
-          }
+          if (c < 0 || c >= t_fld - 1) { fold(fld); ++fld; t_fld = item_step(item_t[fld % kItemT]); continue; }
         }
-        TC_CLK(c3);
         // ---- publish the summary of the next finished block (never waits for a decision on itself)
         if (pub < ntot && pub < n_lim && pub - fld < NP) {
           if (!pub_ready) {
@@ -636,9 +621,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
             pub_ready = (fld == pub) ? mbar_try_wait(pvb, par) : mbar_test_wait(pvb, par);
             if (pub_ready) { t_pub = item_step(item_t[pub % kItemT]); if (tid == 0) TC_TRACE(trf, 7, pub, 0); }
           }
-          TC_CLK(c4);
           if (pub_ready && c < 0) { ++pub; pub_ready = false; continue; }   // fired: an unpublished step lies beyond t*
-          if (pub_ready && (c >= t_pub - M || TC_DBG(4))) {   // mailbox slot free: step t - M has been scanned
+          if (pub_ready && c >= t_pub - M) {                  // mailbox slot free: step t - M has been scanned
             const int t = t_pub;
             const int slot_i = (t - 1) & (M - 1);
             const uint32_t row0 = mapa(sbase + sm.mbox + static_cast<uint32_t>(slot_i) * kSummaryBytes, 0);
@@ -666,19 +650,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
             if (tid == 0) { TC_TRACE(trf, 4, pub, t); TC_TRACE(trf, 13, t, c < 0 ? 0 : c); }
             if (fld == pub) t_fld = t;
             ++pub; pub_ready = false;
-            TC_CLK(c5); TC_ACC(2, c0, c3); TC_ACC(3, c3, c4); TC_ACC(4, c4, c5);
             continue;
           }
         }
-        TC_CLK(c6); TC_ACC(5, c0, c6);
-        // nothing to do yet: do not take issue slots from the warps this one shares its scheduler with
       }
-#ifdef ART_TRACE
-      if (tid == 0 && p.trace && TC_DBG(64)) {
-        unsigned long long* acc = reinterpret_cast<unsigned long long*>(p.trace + 64);
-        for (int k = 0; k < 6; ++k) { atomicAdd(acc + 2 * k, static_cast<unsigned long long>(clk_acc[k])); atomicAdd(acc + 2 * k + 1, static_cast<unsigned long long>(clk_cnt[k])); }
-      }
-#endif
     }
   } else if (ART && warp == kWarpScan && rank == 0) {
     // ===================================================== A6 + A7 + A9: Algorithm 1 over step summaries
@@ -706,7 +681,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
         n = n > kScanBatch ? kScanBatch : n;
         __syncwarp();                                         // the probing lane's acquire covers the whole warp
       }
-      const int fired = TC_DBG(2) ? -1 : sc.batch(n, lane, p.tau, p.phi, p.patience,
+      const int fired = sc.batch(n, lane, p.tau, p.phi, p.patience,
         [&](int k, bool live, float& mt, float& lt) {
           const uint32_t a = mb_lane + static_cast<uint32_t>((i0 + k) & (M - 1)) * kSummaryBytes;
           const float m_ = lds_f32(a), l_ = lds_f32(a + G * 4u);     // a slot that is not part of the batch
