@@ -68,10 +68,13 @@ static EncodeTiledFn encode_tiled_fn() {
 //   HND cache[page][head][token][d]:  dims (128, 64 tokens, page*Hkv + head)
 //   NHD cache[page][token][head][d]:  dims (128, Hkv, page*64 + token)
 // The outermost extent is not known to the ABI (the cache is the caller's); it is set to 2^30.
-static bool encode_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv);
+static bool encode_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv, bool whole);
 // Encoding a tensor map is a driver call; a decode loop passes the same caches every step, so the last few maps
 // are remembered (keyed by base pointer, layout, Hkv: everything the map depends on).
-static bool make_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv) {
+// whole: one box = the whole 64 x 128 tile of a block (rank 4: [d % 64][token][d / 64][page, head]), so a tile is ONE copy
+// instruction (static-cluster kernel); otherwise rank 3 with a box of 64 x 64 (two copies per tile; persistent kernel)
+static bool make_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv, bool whole = false) {
+  if (whole) layout |= 256;
   struct Entry { const void* base; int layout, Hkv; CUtensorMap tm; };
   static std::mutex mu;
   static Entry cache[8];
@@ -81,15 +84,29 @@ static bool make_cache_map(CUtensorMap* tm, const void* base, int layout, int Hk
     for (int i = 0; i < n; ++i)
       if (cache[i].base == base && cache[i].layout == layout && cache[i].Hkv == Hkv) { *tm = cache[i].tm; return true; }
   }
-  if (!encode_cache_map(tm, base, layout, Hkv)) return false;
+  if (!encode_cache_map(tm, base, layout & 255, Hkv, whole)) return false;
   std::lock_guard<std::mutex> lock(mu);
   cache[next] = Entry{base, layout, Hkv, *tm};
   next = (next + 1) % 8; if (n < 8) ++n;
   return true;
 }
-static bool encode_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv) {
+static bool encode_cache_map(CUtensorMap* tm, const void* base, int layout, int Hkv, bool whole) {
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
+  if (whole) {
+    // shared-memory image = [d / 64][token][64 elements]: the two 64-column halves one after the other, each 64 rows x 128 B
+    cuuint64_t dims[4]; cuuint64_t strides[3]; cuuint32_t box[4] = {64, 64, 2, 1}; cuuint32_t es[4] = {1, 1, 1, 1};
+    if (layout == ART_LAYOUT_HND) {                          // [page * Hkv + head][token][d]
+      dims[0] = 64; dims[1] = 64; dims[2] = 2; dims[3] = 1ull << 30;
+      strides[0] = 256; strides[1] = 128; strides[2] = 256ull * 64;
+    } else {                                                 // [page * 64 + token][head][d]
+      dims[0] = 64; dims[1] = 1ull << 30; dims[2] = 2; dims[3] = static_cast<cuuint64_t>(Hkv);
+      strides[0] = 256ull * Hkv; strides[1] = 128; strides[2] = 256;
+    }
+    return enc(tm, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(base), dims, strides, box, es,
+               CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+               CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  }
   cuuint64_t dims[3]; cuuint64_t strides[2]; cuuint32_t box[3]; cuuint32_t es[3] = {1, 1, 1};
   if (layout == ART_LAYOUT_HND) {
     dims[0] = 128; dims[1] = 64; dims[2] = 1ull << 30;
@@ -397,7 +414,7 @@ static int run(const art_desc_t* d, const void* q, const void* k, const void* v,
       if (workspace && workspace_bytes >= (1u << 20)) { cudaMemsetAsync(workspace, 0, 1u << 20, stream); p.trace = static_cast<uint8_t*>(workspace); }
 #endif
       CUtensorMap tmK, tmV;
-      if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads))
+      if (!make_cache_map(&tmK, k, d->kv_layout, d->num_kv_heads, true) || !make_cache_map(&tmV, v, d->kv_layout, d->num_kv_heads, true))
         return ART_ERR_CUDA;
       const bool mt = p.qlen > 1;
       int r;

@@ -133,6 +133,12 @@ __device__ __forceinline__ void tma_load_box(uint32_t dst, const CUtensorMap* tm
   asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %4}], [%5];"
                :: "r"(dst), "l"(tm), "r"(c0), "r"(c1), "r"(c2), "r"(bar) : "memory");
 }
+// a whole 64 x 128 tile with ONE instruction (rank-4 map [d % 64][token][d / 64][page, head]; the image in shared memory is the
+// two 64-column boxes one after the other): HND (0, 0, 0, page * Hkv + head), NHD (0, page * 64, 0, head)
+__device__ __forceinline__ void tma_load_tile(uint32_t dst, const CUtensorMap* tm, int ca, int cb, uint32_t bar) {
+  asm volatile("cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3, %2, %4}], [%5];"
+               :: "r"(dst), "l"(tm), "r"(0), "r"(ca), "r"(cb), "r"(bar) : "memory");
+}
 __device__ __forceinline__ void tmem_alloc(uint32_t smem_dst, uint32_t ncols) {
   asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" :: "r"(smem_dst), "r"(ncols) : "memory");
   asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
@@ -377,7 +383,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
           if (mask) {
             const int page = p.block_table[static_cast<int64_t>(b) * p.max_blocks + blk];
             if (p.layout == ART_LAYOUT_HND) { c1 = 0; c2 = page * p.Hkv + g; }     // [page*Hkv + head][token][d]
-            else { c1 = g; c2 = page * kBlockTokens; }                             // [page*64 + token][head][d]
+            else { c1 = page * kBlockTokens; c2 = g; }                             // [page*64 + token][head][d]
           }
         }
         const int cnt = min(32, n_c - i0);
@@ -399,10 +405,8 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
               mbar_arrive(fb);                                 // nothing to load: an all-masked step
             } else {
               mbar_arrive_expect_tx(fb, kStageBytes);
-              tma_load_box(dst, &tmK, 0, c1_k, c2_k, fb);
-              tma_load_box(dst + kBoxBytes, &tmK, 64, c1_k, c2_k, fb);
-              tma_load_box(dst + 2 * kBoxBytes, &tmV, 0, c1_k, c2_k, fb);
-              tma_load_box(dst + 3 * kBoxBytes, &tmV, 64, c1_k, c2_k, fb);
+              tma_load_tile(dst, &tmK, c1_k, c2_k, fb);
+              tma_load_tile(dst + 2 * kBoxBytes, &tmV, c1_k, c2_k, fb);
             }
           }
           if (mask_k != 0ull) ++loaded;
