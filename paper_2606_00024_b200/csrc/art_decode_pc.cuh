@@ -1,7 +1,8 @@
 // ART decode attention, bf16 KV / head_dim 128, DETECTOR OFF: persistent clusters with run-time scheduling
-// (tcgen05 + TMEM + TMA).  Chosen by the host when the groups are many and short (they do not even fit one two-CTA
-// cluster each: configs[3]), where one short-lived cluster per group would run in several waves, each CTA paying for
-// its own start-up (tensor-memory allocation, cluster barriers, Q staging) and tail.
+// (tcgen05 + TMEM + TMA).  Runs when the caller asks for it (art_desc_t.split < 0) and behind
+// art_decode_attention_off_static.  Built for many short groups (configs[3]), where one short-lived cluster per group runs
+// in several waves, each CTA paying for its own start-up (tensor-memory allocation, cluster barriers, Q staging) and
+// tail; since the MMA operand traffic was halved the static one-CTA clusters are as fast there.
 //
 // The grid is NC thread-block clusters of CL CTAs (two CTAs per SM), launched once and resident for the whole call.
 // Cluster c owns the query groups c, c + NC, c + 2 NC, ...  Nothing inside a cluster is bound:
@@ -21,7 +22,7 @@
 //
 // With the detector ON the library always uses the static clusters of art_decode_tc.cuh: three persistent variants
 // were built and measured in round 2 (summaries pulled over DSMEM, pushed into a home mailbox, scanned by one or by
-// four warps); none came within 25 % of the static clusters (DESIGN.md section 11 has the numbers and the reasons).
+// four warps); none came within 25 % of the static clusters (DESIGN.md section 6.5.2 has the numbers and the reasons).
 #pragma once
 #include "art_decode_tc.cuh"
 

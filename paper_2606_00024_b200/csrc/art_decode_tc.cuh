@@ -6,9 +6,9 @@
 // CTA one 64-token KV block is one pipeline item, handled by specialised warps that meet only through
 // mbarriers, each warp waiting on ONE barrier at a time:
 //
-//   producer (warp 0)      A1/A2  resolves block -> page, issues 4 TMA tensor boxes (K, V: two 64-column
-//                                 halves each, 128-byte swizzle) into the ring of stages
-//   S-MMA    (warp 1, 1 thr) A3   S[token, head] = K_t . Q^T : tcgen05.mma M128 N16 K16, ONE per k-step: the 64
+//   producer (warp 8)      A1/A2  resolves block -> page, issues 2 TMA tensor copies (one per tile: rank-4 map, the image
+//                                 in shared memory is two 64-column boxes, 128-byte swizzle) into the ring of stages
+//   S-MMA    (warp 9, 1 thr) A3   S[token, head] = K_t . Q^T : tcgen05.mma M128 N16 K16, ONE per k-step: the 64
 //                                 tokens are M rows 0-63 (even blocks; TMEM lanes 0-63) or rows 64-127 (odd
 //                                 blocks: the operand starts 64 rows below the tile; lanes 64-127).  What an MMA
 //                                 costs here is reading its A operand (128 rows x 32 B) from shared memory, so
@@ -19,13 +19,13 @@
 //                                 maximum (the warps are stateless), split into bf16 hi + lo (~16 mantissa
 //                                 bits, so the probe of P~V_t is accurate to ~1e-5 and the criterion does not
 //                                 flip) and written to shared memory as the B operand of the P.V MMA
-//   PV-MMA   (warp 3, 1 thr) A5   PV[d, head] = V_t^T . P^T : tcgen05.mma M128 N16 K16 x 4, N = (hi of 8 heads | lo of 8 heads)
-//   fold     (warps 8-11)  A5/A6  one thread per output coordinate: tcgen05.ld of P~V_t; publishes the step
+//   PV-MMA   (warp 10, 1 thr) A5   PV[d, head] = V_t^T . P^T : tcgen05.mma M128 N16 K16 x 4, N = (hi of 8 heads | lo of 8 heads)
+//   fold     (warps 0-3)   A5/A6  one thread per output coordinate: tcgen05.ld of P~V_t; publishes the step
 //                                 summary (m_blk, block sum, probe components of P~V_t) to the cluster
 //                                 leader's mailbox (st.async + mbarrier complete_tx, no fences) and merges
 //                                 P~V_t into the running (m, l, acc) only once the leader has decided that
 //                                 step t <= t*
-//   scan     (warp 2, leader CTA)  A6/A7/A9  replays Algorithm 1 (Eq. 2-3) sequentially
+//   scan     (warp 11, leader CTA) A6/A7/A9  replays Algorithm 1 (Eq. 2-3) sequentially
 //                                 over the step summaries (art_scan.cuh), broadcasts progress / t*
 //
 // The block-local P~V_t of up to 8 steps per CTA wait UNFOLDED in tensor memory, so loads, MMAs and

@@ -6,7 +6,7 @@
 // order here, but the walk is not inherently serial: only the short recurrence
 //     x^(t) = x^(t-1) + (l_t / A_t) (u^(t)[idx] - x^(t-1))
 // is carried from step to step (an affine map of x, so a run of steps could also be composed as a parallel prefix:
-// DESIGN.md section 11, lead 1, has the measurement of that variant) and the patience counter is a walk over bits;
+// DESIGN.md section 11, lead 2, has the measurement of that variant) and the patience counter is a walk over bits;
 // everything else (norms, cross-lane sums, sqrt, divide, compare) is independent per step.  The warp therefore takes a BATCH of up to kScanBatch consecutive steps whose
 // summaries have arrived, runs the recurrence over them back to back, reduces the 4 x batch partial sums
 // with one transposing butterfly (each lane ends up owning one step), evaluates Eq. 2 for all steps of
