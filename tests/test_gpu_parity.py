@@ -240,6 +240,26 @@ def test_error_codes_on_device():
     assert a.art_query_split(a.make_desc(w, split=a.art_split_persistent(3)), False) == 3
 
 
+def test_split_zero_runs_static_clusters_and_is_bit_reproducible():
+    """include/art_decode.h: split = 0 always runs static clusters (persistent clusters only for split < 0), also for
+    many short groups without a cluster of two each; with static clusters `out` and `stop_block` are bit-reproducible
+    from run to run, detector on and off (steps dealt round-robin, merged in order, combined in rank order)."""
+    a = art()
+    many = gen.config(3, scale=1 / 16, batch=48).to("cuda")          # 384 groups: more than 296 one-CTA slots
+    d0 = a.make_desc(many)
+    assert a.art_query_clusters(d0, False) == 0 and a.art_query_split(d0, False) == 1
+    assert a.art_query_clusters(a.make_desc(many, split=a.ART_SPLIT_DYNAMIC), False) >= 1
+    for w, kw in ((many, {}), (gen.config(1, scale=1 / 8, batch=2, recency_decay=(0.2, 1.0)).to("cuda"), {"tau": 1e-3})):
+        for art_on in (True, False):
+            runs = []
+            for _ in range(3):
+                out, stop, _ = a.run_workload(w, art=art_on, **(kw if art_on else {}))
+                torch.cuda.synchronize()
+                runs.append((out.clone(), stop.clone()))
+            for out, stop in runs[1:]:
+                assert torch.equal(out, runs[0][0]) and torch.equal(stop, runs[0][1]), (w.name, art_on)
+
+
 def test_sm_scale_override():
     """desc.sm_scale > 0 replaces 1/sqrt(d) (Eq. 1, R11) on every path."""
     a = art()
