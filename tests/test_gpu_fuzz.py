@@ -1,6 +1,10 @@
 """-m gpu: seeded random shapes / policies / thresholds / schedules against the fp64 oracle.  Every case goes
 through the same check as the hand-written parity tests (stop blocks exact on non-fragile groups, outputs within
-tolerance, loaded >= processed)."""
+tolerance, loaded >= processed).  ART_FUZZ_EXTRA=N adds N further seeds to each of the two families (a sweep to run by
+hand after a kernel change: `ART_FUZZ_EXTRA=1500 python -m pytest tests/test_gpu_fuzz.py -m gpu -x -q`; the default suite
+runs the 48 + 32 committed seeds only)."""
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -73,3 +77,18 @@ def test_random_multi_token_case(seed):
     w, th, split = random_multi_token_case(seed)
     check(w, split=split, **th)
     check(w, art_on=False, split=split)
+
+
+EXTRA = int(os.environ.get("ART_FUZZ_EXTRA", "0"))
+
+
+@pytest.mark.skipif(EXTRA == 0, reason="ART_FUZZ_EXTRA not set")
+@pytest.mark.parametrize("seed", range(48, 48 + max(EXTRA, 1)))
+def test_random_case_extra(seed):
+    test_random_case(seed)
+
+
+@pytest.mark.skipif(EXTRA == 0, reason="ART_FUZZ_EXTRA not set")
+@pytest.mark.parametrize("seed", range(32, 32 + max(EXTRA, 1)))
+def test_random_multi_token_case_extra(seed):
+    test_random_multi_token_case(seed)
