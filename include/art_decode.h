@@ -35,7 +35,8 @@
 extern "C" {
 #endif
 
-#define ART_VERSION 121          /* 0.2.1: art_decode_attention_off_static (no caller workspace); 0.2.0: art_desc_t.num_pages,
+#define ART_VERSION 122          /* 0.2.2: split = 0 always runs static clusters, which are bit-reproducible (same ABI);
+                                    0.2.1: art_decode_attention_off_static (no caller workspace); 0.2.0: art_desc_t.num_pages,
                                     ART_SPLIT_PERSISTENT, art_query_clusters, art_hbm_read_probe */
 #define ART_BLOCK_TOKENS 64      /* n: tokens per KV block = per cache page */
 #define ART_SPLIT_DYNAMIC (-1)   /* art_desc_t.split: persistent clusters, cluster size chosen by the library (BF16, detector

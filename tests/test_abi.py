@@ -32,7 +32,7 @@ def test_every_declared_symbol_is_exported(art):
             "art_static_scratch_needed"} <= set(syms)
     for s in syms:
         assert hasattr(lib, s), s
-    assert art.art_version() == 121
+    assert art.art_version() == 122
     assert "NULL" in art.art_status_string(-1) and art.art_status_string(0) == "ok"
 
 
