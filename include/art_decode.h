@@ -218,7 +218,9 @@ int art_decode_attention_host(const art_desc_t* desc, const void* q_host, const 
  *                             ties -> lower block index first (reading R10); eligible_counts[b, g] = their number
  * The outputs are what art_decode_attention takes with policy == LIST.  Uses desc->{batch, num_q_heads,
  * num_kv_heads, head_dim, block_tokens, dtype, kv_layout, max_blocks_per_seq (<= 4096), max_eligible (row stride
- * of eligible_blocks, >= top_k)}; q_len must be 0 or 1.  q, k_cache, block_table, seq_lens as above; block_scores DEVICE float32
+ * of eligible_blocks, >= top_k), q_len}.  With q_len = m > 1 (q is [B, m, Hq, d]) the LAST query token scores the blocks: the
+ * policy's eligible set and order are the group's, computed as for the last token (reading R15).  q, k_cache,
+ * block_table, seq_lens as above; block_scores DEVICE float32
  * [B, Hkv, max_blocks_per_seq]; eligible_blocks DEVICE int32 [B, Hkv, max_eligible]; eligible_counts DEVICE
  * int32 [B, Hkv].  Enqueues two kernels on cuda_stream and returns.  Entries beyond the count are not written.
  */

@@ -596,7 +596,7 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
                     int32_t* eligible_counts, void* cuda_stream) {
   if (!d || !q || !k_cache || !block_table || !seq_lens || !block_scores || !eligible_blocks || !eligible_counts) return ART_ERR_NULL;
   if (d->batch < 0 || d->num_q_heads <= 0 || d->num_kv_heads <= 0 || d->num_q_heads % d->num_kv_heads) return ART_ERR_SHAPE;
-  if (d->num_q_heads / d->num_kv_heads > 8 || d->q_len > 1) return ART_ERR_SHAPE;    // scores are defined for one query token
+  if (d->num_q_heads / d->num_kv_heads > 8 || d->q_len < 0 || art::rows_of(d) > 8) return ART_ERR_SHAPE;   // q_len = m: the last token scores (R15)
   const int G = art::padded_group(d->num_q_heads / d->num_kv_heads);
   if (d->block_tokens != ART_BLOCK_TOKENS) return ART_ERR_SHAPE;
   if (!((d->dtype == ART_DTYPE_F32 && d->head_dim == 64) || (d->dtype == ART_DTYPE_BF16 && d->head_dim == 128))) return ART_ERR_DTYPE;
@@ -613,7 +613,7 @@ int art_topk_blocks(const art_desc_t* d, const void* q, const void* k_cache, con
   art::policy::ScoreParams sp = {};
   sp.q = q; sp.k = static_cast<const uint8_t*>(k_cache); sp.block_table = block_table; sp.seq_lens = seq_lens;
   sp.scores = block_scores; sp.batch = d->batch; sp.Hq = d->num_q_heads; sp.Hkv = d->num_kv_heads; sp.Gr = d->num_q_heads / d->num_kv_heads;
-  sp.max_blocks = d->max_blocks_per_seq; sp.layout = d->kv_layout;
+  sp.max_blocks = d->max_blocks_per_seq; sp.layout = d->kv_layout; sp.qlen = art::qlen_of(d);
   const int64_t row = art::kRowBytes;
   if (d->kv_layout == ART_LAYOUT_HND) { sp.token_stride = row; sp.head_stride = row * art::kBlockTokens; sp.page_stride = sp.head_stride * d->num_kv_heads; }
   else { sp.head_stride = row; sp.token_stride = row * d->num_kv_heads; sp.page_stride = sp.token_stride * art::kBlockTokens; }

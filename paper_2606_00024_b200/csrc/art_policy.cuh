@@ -22,6 +22,7 @@ struct ScoreParams {
   const int32_t* seq_lens;
   float* scores;                               // [B, Hkv, max_blocks]
   int32_t batch, Hq, Hkv, Gr, max_blocks, layout;   // Gr: real heads per group (the template G is its power-of-two ceiling)
+  int32_t qlen;                                // query tokens per sequence (R15): the LAST one scores the blocks
   int64_t page_stride, head_stride, token_stride;   // bytes
 };
 
@@ -61,7 +62,8 @@ __global__ void __launch_bounds__(kScoreWarps * 32) art_block_scores_kernel(cons
   float qs[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) qs[e] = 0.f;
-  const T* qp = reinterpret_cast<const T*>(p.q) + (static_cast<int64_t>(b) * p.Hq + g * p.Gr) * D;
+  // q is [B, m, Hq, D]; the policy is the group's, computed as for the last query token (reading R15)
+  const T* qp = reinterpret_cast<const T*>(p.q) + ((static_cast<int64_t>(b) * p.qlen + (p.qlen - 1)) * p.Hq + g * p.Gr) * D;
 #pragma unroll
   for (int h = 0; h < G; ++h) {
     if (h >= p.Gr) break;

@@ -121,6 +121,40 @@ def test_full_size_config2_scores_sampled():
     torch.cuda.empty_cache()
 
 
+@pytest.mark.parametrize("m,G", [(2, 4), (4, 2), (8, 1), (3, 2)])
+def test_multi_token_queries_are_scored_by_their_last_token(m, G):
+    """Reading R15: with q_len = m the policy's eligible set and order are the group's, computed as for the LAST query
+    token.  art_topk_blocks on q [B, m, Hq, d] == the oracle on q[:, m - 1] == art_topk_blocks on that token alone
+    (bit for bit), and the device-built list feeds the multi-token attention call."""
+    a = art()
+    base = gen.make_workload("pm", seed=77 + m, batch=2, num_q_heads=G * 2, num_kv_heads=2, head_dim=128,
+                             seq_lens=[1500, 777], planted_frac=0.01, sink_plant=4, recency_decay=(0.2, 1.0))
+    w = gen.with_query_tokens(base, m, seed=300 + m)
+    last = replace(w, q=w.q[:, m - 1].contiguous())
+    top_k = 9
+    s_ref = ao.block_scores_oracle(np64(last.q), np64(w.k_cache), w.block_table.numpy(), w.seq_lens.numpy(),
+                                   num_kv_heads=w.num_kv_heads, layout=w.layout)
+    l_ref, c_ref = ao.topk_blocks_oracle(s_ref, w.seq_lens.numpy(), top_k)
+    s_m, l_m, c_m = gpu_lists(w, top_k)
+    s_1, l_1, c_1 = gpu_lists(last, top_k)
+    assert np.array_equal(s_m, s_1) and np.array_equal(c_m, c_1)
+    for b in range(w.batch):
+        for g in range(w.num_kv_heads):
+            assert np.array_equal(l_m[b, g, :c_m[b, g]], l_1[b, g, :c_1[b, g]])
+    fin = np.isfinite(s_ref)
+    assert np.array_equal(c_m, c_ref) and np.abs(s_m[fin] - s_ref[fin]).max() <= 2e-5 * max(1.0, float(np.abs(s_ref[fin]).max()))
+    # the device-built list through the multi-token attention kernel, against the oracle on the same list
+    wl = replace(w, policy=gen.POLICY_LIST, eligible_blocks=torch.from_numpy(l_m.astype(np.int32)),
+                 eligible_counts=torch.from_numpy(c_m.astype(np.int32)))
+    wc = wl.to("cuda")
+    for art_on in (True, False):
+        out, stop, _ = a.run_workload(wc, art=art_on, **({"tau": 1e-3} if art_on else {}))
+        torch.cuda.synchronize()
+        over = {"tau": float(np.float32(1e-3))} if art_on else {}
+        rep = compare(wl, out, stop, art=art_on, oracle_over=over)
+        assert rep.ok(OUT_TOL[wl.dtype]), rep.summary()
+
+
 def test_error_codes():
     a = art()
     w = gen.make_workload("e", seed=1, batch=1, num_q_heads=4, num_kv_heads=1, head_dim=128, seq_lens=[300]).to("cuda")
