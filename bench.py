@@ -489,7 +489,7 @@ def main():
     ap.add_argument("--study", action="store_true", help="probe-vs-full, ablation and sensitivity sweeps (SURVEY 8(f))")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-parity", action="store_true", help="--report without the oracle columns (timing only)")
-    ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default, -1 = dynamic scheduler)")
+    ap.add_argument("--split", type=int, default=0, help="cluster size for --arm / --report (0 = library default = static clusters, -1 - cl = persistent clusters of cl CTAs, detector off only)")
     ap.add_argument("--arm", default=None, choices=["on", "off", "pinf", "R_on", "R_off"],
                     help="time ONLY this arm of one config (short command for ncu captures; prints a small JSON line)")
     ap.add_argument("--q-len", type=int, default=1, help="--arm only: m query tokens per sequence (SURVEY 8(f).4; m * G <= 8)")
