@@ -349,12 +349,14 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       if (c >= t - p.run_ahead) return true;
     }
   };
-  // Every issued item runs through all roles (one beyond t* is dropped by the fold warps); a wait can only fail
-  // once the producer has issued its last item (n_lim, fewer if Algorithm 1 fires).
-  auto wait_item = [&](uint32_t baddr, uint32_t parity, int i) -> bool {
-    if constexpr (!ART) { mbar_wait(baddr, parity); return true; }          // detector off: every item arrives
-    while (!mbar_try_wait(baddr, parity)) { if (i >= ld_volatile_s32(a_ntotal)) return false; }
-    return true;
+  // Every issued item runs through all roles (one beyond t* is dropped by the fold warps), so every wait below is a plain
+  // blocking wait.  When Algorithm 1 fires before the producer has issued its n_lim items, the producer publishes the number it
+  // did issue (n_total) and sends ONE more, empty item down the pipeline (END): a role that wakes up for item i >= n_total
+  // hands the wake-up on to the next role and leaves.  Nothing polls, and the roles leave as soon as the last real item is
+  // through (a wait that also polled "no further item" noticed it only when its try_wait timed out, microseconds later).
+  auto is_end = [&](int i) -> bool {
+    if constexpr (!ART) return false;
+    return i >= ld_volatile_s32(a_ntotal);
   };
 
   // fold warps: this thread's output coordinate and the running (un-normalised) state; read by the epilogue
@@ -422,6 +424,13 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
 #endif
     // drain: tensor copies still in flight must land before the CTA reuses the ring or exits (H5)
     for (int j = max(0, it_issued - S); j < it_issued; ++j) mbar_wait(bar(sm.full0 + j % S), (j / S) & 1);
+    // END: stopped early, the other roles wait for item it_issued.  It is issued like an all-masked step (its stage must be free:
+    // every role has then seen the stage's previous phase), after n_total says that it is not a real one.
+    if (ART && it_issued < n_c) {
+      if (it_issued >= S) mbar_wait(bar(sm.empty0 + stage), ph ^ 1u);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(sm.full0 + stage));
+    }
   } else if (warp == kWarpMmaS) {
     // ===================================================== A3: S = K_t Q^T, rows = tokens, columns = heads
     if (lane == 0) {
@@ -432,9 +441,17 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       TC_TRACE_INIT(trm, 3);
       for (int i = 0; i < n_lim; ++i) {
         const int q = i & (NS - 1);
-        if (!wait_item(bar(sm.full0 + st), ph, i)) break;
+        mbar_wait(bar(sm.full0 + st), ph);
+        if (is_end(i)) {                                      // wake both softmax pairs (their next blocks are i and i + 1)
+          for (int j = 0; j < 2; ++j) {
+            const int ii = i + j, qq = ii & (NS - 1);
+            if (ii >= NS) mbar_wait(bar(sm.sfree0 + qq), ((ii / NS) - 1) & 1);
+            umma_commit(bar(sm.sfull0 + qq));
+          }
+          break;
+        }
         TC_TRACE(trm, 2, i, 0);
-        if (i >= NS && !wait_item(bar(sm.sfree0 + q), ((i / NS) - 1) & 1, i)) break;
+        if (i >= NS) mbar_wait(bar(sm.sfree0 + q), ((i / NS) - 1) & 1);
         TC_TRACE(trm, 10, i, 0);
         tc_fence_after();
         // M = 128 rows are read starting at the tile (even blocks: tokens 0-63 -> TMEM lanes 0-63) or 64 token rows
@@ -465,9 +482,10 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       TC_TRACE_INIT(trv, 5);
       for (int i = 0; i < n_lim; ++i) {
         const int ps = i & (NP - 1);
-        if (!wait_item(bar(sm.pfull0 + st), ph, i)) break;
+        mbar_wait(bar(sm.pfull0 + st), ph);
+        if (is_end(i)) break;
         TC_TRACE(trv, 6, i, 0);
-        if (i >= NP && !wait_item(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1, i)) break;
+        if (i >= NP) mbar_wait(bar(sm.pvfree0 + ps), ((i / NP) - 1) & 1);
         TC_TRACE(trv, 11, i, 0);
         tc_fence_after();
         const uint32_t vt = sbase + sm.ring + st * kStageBytes + 2 * kBoxBytes;
@@ -493,7 +511,14 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     TC_TRACE_INIT(trx, 4);
     for (int i = pair; i < n_lim; i += 2) {
       const int sslot = i & (NS - 1);
-      if (!wait_item(bar(sm.sfull0 + sslot), (i / NS) & 1, i)) break;
+      mbar_wait(bar(sm.sfull0 + sslot), (i / NS) & 1);
+      if constexpr (ART) {
+        const int nt = ld_volatile_s32(a_ntotal);
+        if (i >= nt) {                                        // END: the pair that owns the END item hands it on to the P.V issuer
+          if (i == nt) mbar_arrive(bar(sm.pfull0 + st));
+          break;
+        }
+      }
       if (q == 0 && lane == 0) TC_TRACE(trx, 3, i, 0);
       tc_fence_after();
       float sv[G];
@@ -503,7 +528,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(sm.sfree0 + sslot));
       // P^T buffer i & 1 is read by the P.V MMA of block i - 2: wait until that one is complete
-      if (kTwoPBufs && i >= 2 && !wait_item(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1, i)) break;
+      if (kTwoPBufs && i >= 2) mbar_wait(bar(sm.pvfull0 + ((i - 2) & (NP - 1))), ((i - 2) / NP) & 1);
       const unsigned long long vmask = sinfo[st];             // written before the loads the S MMA waited for
       const bool v0 = (vmask >> tok) & 1ull;
       float mb[G];
@@ -598,7 +623,7 @@ art_decode_tc_kernel(const Params p, const __grid_constant__ CUtensorMap tmK, co
     };
     if constexpr (!ART) {
       for (int i = 0; i < n_lim; ++i) {
-        if (!wait_item(bar(sm.pvfull0 + (i & (NP - 1))), (i / NP) & 1, i)) break;
+        mbar_wait(bar(sm.pvfull0 + (i & (NP - 1))), (i / NP) & 1);
         fold(i);
       }
     } else {
